@@ -1,0 +1,302 @@
+"""Seeded synthetic workloads shaped like the paper's tests (BASELINE.json configs 1-5).
+
+This module is the ONLY thing the CUDA path and the CPU oracle share.  It holds the input
+recipes (initial primitives on packed blocks with ghosts already filled, parameter
+dictionaries) and none of the method's arithmetic: no fluxes, no reconstruction, no
+con2prim, no wave speeds.  The two geometric formulas it needs to *shape* the Kerr-Schild
+inputs (the Kerr-Schild radius r and sqrt(gamma)=sqrt(1+2H), used to place the excised
+region and to turn the divergence-free densitised field into the primitive B) are part of
+the recipe stated in DESIGN.md section 4.
+
+Layout of every field: [block][var][k][j][i], i fastest, fp64, var order
+(rho, u~1, u~2, u~3, u=rho*eps, B1, B2, B3)  (Eq.13).
+Block id = (bz*nby + by)*nbx + bx.  A dimension with one zone in total is inactive and has
+no ghost zones.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+NV = 8
+SEED0 = 241009146
+
+MINKOWSKI, KERR_SCHILD = 0, 1
+RECON_CONST, RECON_PLM_MINMOD, RECON_PLM_MC, RECON_WENO5Z = 0, 1, 2, 3
+RIEMANN_LLF, RIEMANN_HLL = 0, 1
+BC_PERIODIC, BC_OUTFLOW = 0, 1
+
+
+def default_params(**kw):
+    p = dict(
+        metric=MINKOWSKI, bh_mass=1.0, bh_spin=0.0, r_excise=0.0,
+        nbx=1, nby=1, nbz=1, nx=1, ny=1, nz=1, ng=4,
+        xmin=(0.0, 0.0, 0.0), xmax=(1.0, 1.0, 1.0),
+        bc=((BC_PERIODIC, BC_PERIODIC),) * 3,
+        gamma_ad=5.0 / 3.0, recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL, use_ct=1,
+        rho_floor=1e-10, eps_floor=1e-10, w_max=50.0, c2p_tol=1e-15, c2p_maxit=64,
+    )
+    p.update(kw)
+    return p
+
+
+# --------------------------------------------------------------------------- layout helpers
+def ghosts(p):
+    """Ghost depth per dimension (0 in an inactive dimension)."""
+    tot = (p["nbx"] * p["nx"], p["nby"] * p["ny"], p["nbz"] * p["nz"])
+    return tuple(p["ng"] if t > 1 else 0 for t in tot)
+
+
+def alloc_shape(p):
+    gx, gy, gz = ghosts(p)
+    nb = p["nbx"] * p["nby"] * p["nbz"]
+    return (nb, NV, p["nz"] + 2 * gz, p["ny"] + 2 * gy, p["nx"] + 2 * gx)
+
+
+def n_zones(p):
+    return p["nbx"] * p["nx"] * p["nby"] * p["ny"] * p["nbz"] * p["nz"]
+
+
+def cell_centres(p):
+    """Global interior cell-centre coordinates (x[i], y[j], z[k])."""
+    out = []
+    for d, (nb, n) in enumerate(((p["nbx"], p["nx"]), (p["nby"], p["ny"]), (p["nbz"], p["nz"]))):
+        N = nb * n
+        dx = (p["xmax"][d] - p["xmin"][d]) / N
+        out.append(p["xmin"][d] + (np.arange(N) + 0.5) * dx)
+    return out
+
+
+def node_coords(p):
+    out = []
+    for d, (nb, n) in enumerate(((p["nbx"], p["nx"]), (p["nby"], p["ny"]), (p["nbz"], p["nz"]))):
+        N = nb * n
+        dx = (p["xmax"][d] - p["xmin"][d]) / N
+        out.append(p["xmin"][d] + np.arange(N + 1) * dx)
+    return out
+
+
+def pad_global(p, q):
+    """q: [NV, Nz, Ny, Nx] global interior -> global array with ghosts, filled x then y then z
+    (periodic: wrap; outflow: copy of the nearest interior cell)."""
+    gx, gy, gz = ghosts(p)
+    for axis, g, d in ((3, gx, 0), (2, gy, 1), (1, gz, 2)):
+        if g == 0:
+            continue
+        lo, hi = p["bc"][d]
+        if lo != hi:
+            raise ValueError("mixed boundary conditions on one axis are not used by any workload")
+        w = [(0, 0)] * 4
+        w[axis] = (g, g)
+        q = np.pad(q, w, mode="wrap" if lo == BC_PERIODIC else "edge")
+    return q
+
+
+def to_blocks(p, qpad):
+    """Cut a global padded array [NV, Nz+2gz, Ny+2gy, Nx+2gx] into packed blocks with ghosts."""
+    gx, gy, gz = ghosts(p)
+    nx, ny, nz = p["nx"], p["ny"], p["nz"]
+    out = np.empty(alloc_shape(p), dtype=np.float64)
+    for bz in range(p["nbz"]):
+        for by in range(p["nby"]):
+            for bx in range(p["nbx"]):
+                b = (bz * p["nby"] + by) * p["nbx"] + bx
+                out[b] = qpad[:, bz * nz: bz * nz + nz + 2 * gz,
+                              by * ny: by * ny + ny + 2 * gy,
+                              bx * nx: bx * nx + nx + 2 * gx]
+    return out
+
+
+def from_blocks(p, qb):
+    """Packed blocks -> global interior array [nvar, Nz, Ny, Nx] (ghosts dropped)."""
+    gx, gy, gz = ghosts(p)
+    nx, ny, nz = p["nx"], p["ny"], p["nz"]
+    qb = np.asarray(qb)
+    nvar = qb.shape[1]
+    out = np.empty((nvar, p["nbz"] * nz, p["nby"] * ny, p["nbx"] * nx), dtype=qb.dtype)
+    for bz in range(p["nbz"]):
+        for by in range(p["nby"]):
+            for bx in range(p["nbx"]):
+                b = (bz * p["nby"] + by) * p["nbx"] + bx
+                out[:, bz * nz:(bz + 1) * nz, by * ny:(by + 1) * ny, bx * nx:(bx + 1) * nx] = \
+                    qb[b][:, gz: gz + nz, gy: gy + ny, gx: gx + nx]
+    return out
+
+
+def finish(p, q):
+    """Global interior primitives -> packed blocks with ghosts."""
+    return np.ascontiguousarray(to_blocks(p, pad_global(p, np.ascontiguousarray(q))))
+
+
+# --------------------------------------------------------------------------- recipe helpers
+def node_curl(Ax, Ay, Az, dx, dy, dz):
+    """Cell-centred densitised field from nodal vector potential, arrays [Nz+1, Ny+1, Nx+1]:
+    B~x = d_y(avg_xz Az) - d_z(avg_xy Ay) etc.  Difference and average operators commute, so
+    the corner-centred divergence of the result vanishes to round-off."""
+    def mu(a, ax):
+        s0 = [slice(None)] * 3; s1 = [slice(None)] * 3
+        s0[ax] = slice(0, -1); s1[ax] = slice(1, None)
+        return 0.5 * (a[tuple(s0)] + a[tuple(s1)])
+
+    def de(a, ax, h):
+        s0 = [slice(None)] * 3; s1 = [slice(None)] * 3
+        s0[ax] = slice(0, -1); s1[ax] = slice(1, None)
+        return (a[tuple(s1)] - a[tuple(s0)]) / h
+    X, Y, Z = 2, 1, 0  # array axes of x, y, z
+    Bx = de(mu(mu(Az, X), Z), Y, dy) - de(mu(mu(Ay, X), Y), Z, dz)
+    By = de(mu(mu(Ax, X), Y), Z, dz) - de(mu(mu(Az, Y), Z), X, dx)
+    Bz = de(mu(mu(Ay, Y), Z), X, dx) - de(mu(mu(Ax, X), Z), Y, dy)
+    return Bx, By, Bz
+
+
+def ks_radius(x, y, z, a):
+    R2 = x * x + y * y + z * z
+    t = R2 - a * a
+    return np.sqrt(0.5 * (t + np.sqrt(t * t + 4.0 * a * a * z * z)))
+
+
+def ks_sqrt_gamma(x, y, z, M, a):
+    r = ks_radius(x, y, z, a)
+    H = M * r ** 3 / (r ** 4 + a * a * z * z)
+    return np.sqrt(1.0 + 2.0 * H)
+
+
+def band_field(rng, n, kmin=1, kmax=8, slope=-2.0):
+    """Real periodic Gaussian field on an n^3 lattice: integer wavevectors kmin<=|k|<=kmax,
+    amplitude ~ |k|^slope, random phases, normalised to unit variance."""
+    kx = np.fft.fftfreq(n, 1.0 / n)
+    kz = np.fft.rfftfreq(n, 1.0 / n)
+    K2 = kx[:, None, None] ** 2 + kx[None, :, None] ** 2 + kz[None, None, :] ** 2
+    K = np.sqrt(K2)
+    sel = (K >= kmin) & (K <= kmax)
+    amp = np.zeros_like(K)
+    amp[sel] = K[sel] ** slope
+    ph = rng.uniform(0.0, 2.0 * np.pi, size=K.shape)
+    g = rng.standard_normal(K.shape)
+    f = np.fft.irfftn(amp * g * np.exp(1j * ph), s=(n, n, n), axes=(0, 1, 2))
+    f -= f.mean()
+    f /= f.std()
+    return f
+
+
+def solenoidal_from_potential(a0, a1, a2, n):
+    """curl of a periodic vector field (spectral), arrays indexed [z][y][x]."""
+    k = 2.0 * np.pi * np.fft.fftfreq(n, 1.0 / n)
+    kr = 2.0 * np.pi * np.fft.rfftfreq(n, 1.0 / n)
+    KZ, KY, KX = k[:, None, None], k[None, :, None], kr[None, None, :]
+    fx, fy, fz = (np.fft.rfftn(a) for a in (a0, a1, a2))
+    cx = 1j * (KY * fz - KZ * fy)
+    cy = 1j * (KZ * fx - KX * fz)
+    cz = 1j * (KX * fy - KY * fx)
+    return tuple(np.fft.irfftn(c, s=(n, n, n), axes=(0, 1, 2)) for c in (cx, cy, cz))
+
+
+# --------------------------------------------------------------------------- the five configs
+def shock_tube(n=256):
+    """Config 1: 1-D relativistic MHD shock tube (PAPER.md:443-445 shape; states from BASELINE.json)."""
+    p = default_params(nx=n, ng=2, gamma_ad=2.0, recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL,
+                       bc=((BC_OUTFLOW, BC_OUTFLOW),) * 3, xmin=(0.0, 0.0, 0.0), xmax=(1.0, 1.0, 1.0))
+    x = cell_centres(p)[0]
+    left = x < 0.5
+    q = np.zeros((NV, 1, 1, n))
+    q[0, 0, 0] = np.where(left, 1.0, 0.125)
+    q[4, 0, 0] = np.where(left, 1.0, 0.1) / (p["gamma_ad"] - 1.0)
+    q[5, 0, 0] = 0.5
+    q[6, 0, 0] = np.where(left, 1.0, -1.0)
+    return dict(name="cfg1_shock_tube", params=p, prim=finish(p, q), cfl=0.4, t_end=0.4, steps=None)
+
+
+def periodic_box(n=64, seed=SEED0 + 2, recon=RECON_PLM_MC, riemann=RIEMANN_LLF):
+    """Config 2: 3-D periodic box with small seeded perturbations."""
+    p = default_params(nx=n, ny=n, nz=n, ng=4, gamma_ad=5.0 / 3.0, recon=recon, riemann=riemann)
+    rng = np.random.default_rng(seed)
+    q = np.zeros((NV, n, n, n))
+    q[0] = 1.0 + 1e-3 * rng.uniform(-1, 1, (n, n, n))
+    P = 1.0 + 1e-3 * rng.uniform(-1, 1, (n, n, n))
+    v = (0.1 / np.sqrt(3.0)) * rng.uniform(-1, 1, (3, n, n, n))
+    W = 1.0 / np.sqrt(1.0 - (v ** 2).sum(0))
+    q[1:4] = W * v
+    q[4] = P / (p["gamma_ad"] - 1.0)
+    q[5], q[6], q[7] = 1.0, 0.5, 0.25
+    return dict(name="cfg2_periodic_box", params=p, prim=finish(p, q), cfl=0.4, steps=100)
+
+
+def _torus_prims(p, seed):
+    M, a, gam = p["bh_mass"], p["bh_spin"], p["gamma_ad"]
+    x, y, z = cell_centres(p)
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    rng = np.random.default_rng(seed)
+    shape = X.shape
+    wcyl = np.sqrt(X * X + Y * Y)
+    rho = np.maximum(1e-4, np.exp(-((wcyl - 10.0) ** 2 + Z * Z) / 8.0))
+    P = 0.01 * rho ** gam * (1.0 + 0.02 * rng.uniform(-1, 1, shape))
+    # Keplerian-like azimuthal motion given directly as the primitive u~ (any u~ is subluminal)
+    uK = np.where(rho > 1e-4, np.minimum(0.5, 1.0 / np.sqrt(np.maximum(wcyl, 1e-30))), 0.0)
+    q = np.zeros((NV,) + shape)
+    q[0] = rho
+    q[1] = -uK * Y / np.maximum(wcyl, 1e-30)
+    q[2] = uK * X / np.maximum(wcyl, 1e-30)
+    q[4] = P / (gam - 1.0)
+    # B from nodal A_phi = max(rho - 0.2, 0)
+    xn, yn, zn = node_coords(p)
+    Zn, Yn, Xn = np.meshgrid(zn, yn, xn, indexing="ij")
+    wn2 = np.maximum(Xn * Xn + Yn * Yn, 1e-30)
+    rhon = np.maximum(1e-4, np.exp(-((np.sqrt(wn2) - 10.0) ** 2 + Zn * Zn) / 8.0))
+    Aphi = np.maximum(rhon - 0.2, 0.0)
+    Ax, Ay, Az = -Yn * Aphi / wn2, Xn * Aphi / wn2, np.zeros_like(Aphi)
+    dx = [(p["xmax"][d] - p["xmin"][d]) / N for d, N in enumerate((len(x), len(y), len(z)))]
+    Bx, By, Bz = node_curl(Ax, Ay, Az, *dx)
+    sg = ks_sqrt_gamma(X, Y, Z, M, a)
+    q[5], q[6], q[7] = Bx / sg, By / sg, Bz / sg
+    return q
+
+
+def kerr_schild_torus(n=128, seed=SEED0 + 3, spin=0.9375, half=20.0):
+    """Config 3: single 3-D block in Cartesian Kerr-Schild coordinates, torus-like data."""
+    p = default_params(metric=KERR_SCHILD, bh_mass=1.0, bh_spin=spin, r_excise=2.0,
+                       nx=n, ny=n, nz=n, ng=4, xmin=(-half,) * 3, xmax=(half,) * 3,
+                       bc=((BC_OUTFLOW, BC_OUTFLOW),) * 3, gamma_ad=4.0 / 3.0,
+                       recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL,
+                       rho_floor=1e-6, eps_floor=1e-6, w_max=10.0)
+    q = _torus_prims(p, seed)
+    return dict(name="cfg3_kerr_schild_torus", params=p, prim=finish(p, q), cfl=0.4, steps=50)
+
+
+def turbulence_box(n=256, seed=SEED0 + 4, recon=RECON_WENO5Z, riemann=RIEMANN_HLL):
+    """Config 4: periodic turbulence-like box (the roofline-target workload at n=256)."""
+    p = default_params(nx=n, ny=n, nz=n, ng=4, gamma_ad=5.0 / 3.0, recon=recon, riemann=riemann)
+    rng = np.random.default_rng(seed)
+    kmax = min(8, n // 4)
+    q = np.zeros((NV, n, n, n))
+    q[0] = np.exp(0.5 * band_field(rng, n, 1, kmax))
+    P = np.exp(0.5 * band_field(rng, n, 1, kmax))
+    q[4] = P / (p["gamma_ad"] - 1.0)
+    ux, uy, uz = solenoidal_from_potential(*(band_field(rng, n, 1, kmax) for _ in range(3)), n)
+    rms = np.sqrt(np.mean(ux ** 2 + uy ** 2 + uz ** 2))
+    q[1], q[2], q[3] = (0.3 / rms) * ux, (0.3 / rms) * uy, (0.3 / rms) * uz
+    # nodal vector potential on the periodic node lattice (same lattice shifted by half a cell)
+    A = [np.pad(band_field(rng, n, 1, kmax), ((0, 1),) * 3, mode="wrap") for _ in range(3)]
+    Bx, By, Bz = node_curl(A[0], A[1], A[2], 1.0 / n, 1.0 / n, 1.0 / n)
+    s = np.sqrt(2.0 * P.sum() / (10.0 * (Bx ** 2 + By ** 2 + Bz ** 2).sum()))   # beta = 2P/B^2 = 10
+    q[5], q[6], q[7] = s * Bx, s * By, s * Bz
+    return dict(name="cfg4_turbulence_box", params=p, prim=finish(p, q), cfl=0.4, steps=20)
+
+
+def packed_blocks(nb=(8, 8, 8), n=32, seed=SEED0 + 5, spin=0.5, half=20.0):
+    """Config 5: many small blocks tiling a Kerr-Schild domain (512 x 32^3 at full size)."""
+    half = (half, half, half * nb[2] / nb[0])
+    p = default_params(metric=KERR_SCHILD, bh_mass=1.0, bh_spin=spin, r_excise=2.0,
+                       nbx=nb[0], nby=nb[1], nbz=nb[2], nx=n, ny=n, nz=n, ng=4,
+                       xmin=tuple(-h for h in half), xmax=half,
+                       bc=((BC_OUTFLOW, BC_OUTFLOW),) * 3, gamma_ad=4.0 / 3.0,
+                       recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL,
+                       rho_floor=1e-6, eps_floor=1e-6, w_max=10.0)
+    q = _torus_prims(p, seed)
+    return dict(name="cfg5_packed_blocks", params=p, prim=finish(p, q), cfl=0.4, steps=20)
+
+
+def reblock(p, prim_blocks, nb):
+    """Same global data on a different block decomposition (for the block-invariance pin)."""
+    tot = (p["nbx"] * p["nx"], p["nby"] * p["ny"], p["nbz"] * p["nz"])
+    p2 = dict(p)
+    p2.update(nbx=nb[0], nby=nb[1], nbz=nb[2], nx=tot[0] // nb[0], ny=tot[1] // nb[1], nz=tot[2] // nb[2])
+    return p2, finish(p2, from_blocks(p, prim_blocks))
