@@ -1,0 +1,118 @@
+/* phx.h — C ABI of the B200-native ideal-GRMHD finite-volume hot path (after PHOEBUS, arXiv:2410.09146).
+ *
+ * Every entry point runs hand-written sm_100a CUDA kernels; there is no CPU fallback.  All `d_*`
+ * pointers are DEVICE pointers owned by the caller (16-byte aligned), all `h_*` pointers are HOST
+ * pointers.  `stream` is a cudaStream_t passed as void* (NULL = default stream); every call is
+ * asynchronous on it unless stated otherwise.  Every function returns PHX_OK or an error code and
+ * never throws or aborts; phx_last_error() returns a thread-local message for the last failure.
+ * Numerical trouble is never an error code: it is reported per cell in the mask.
+ *
+ * Field layout (all fp64): [block][var][k][j][i], i fastest, 8 variables, ghosts included.
+ *   primitives  P  = (rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3)            PAPER.md:111-113 (Eq.13)
+ *   conserved   U~ = sqrt(gamma) * (D, S_1, S_2, S_3, tau, B^1, B^2, B^3)           PAPER.md:59-63 (Eq.1-2)
+ * Block id = (bz*nby + by)*nbx + bx.  A dimension with one zone in the whole domain is inactive:
+ * it has no ghost zones and no sweep.  Ghosts of U~ are never read or written.
+ * Mask layout: [block][k][j][i] (uint8, same cell indexing as one variable).
+ */
+#ifndef PHX_H
+#define PHX_H
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct phx_mesh phx_mesh; /* opaque; owns flux scratch, excision flags and reduction scratch on the device */
+
+enum { PHX_OK = 0, PHX_EINVAL = 1, PHX_ECUDA = 2, PHX_ENOMEM = 3, PHX_EUNSUPPORTED = 4 };
+enum { PHX_MINKOWSKI = 0, PHX_KERR_SCHILD = 1 }; /* Cartesian Kerr-Schild, ingoing (analytic metrics) */
+enum { PHX_RECON_CONST = 0, PHX_RECON_PLM_MINMOD = 1, PHX_RECON_PLM_MC = 2, PHX_RECON_WENO5Z = 3 }; /* PAPER.md:275, App.B */
+enum { PHX_RIEMANN_LLF = 0, PHX_RIEMANN_HLL = 1 };
+enum { PHX_BC_PERIODIC = 0, PHX_BC_OUTFLOW = 1 };
+/* con2prim / floor mask bits */
+enum {
+  PHX_M_RHO_FLOOR = 1, PHX_M_EPS_FLOOR = 2, PHX_M_EPS_CLIPPED = 4, PHX_M_W_CEIL = 8,
+  PHX_M_NOCONV = 16, PHX_M_BAD_INPUT = 32, PHX_M_EXCISED = 64
+};
+
+typedef struct {
+  int metric;
+  double bh_mass, bh_spin, r_excise; /* Kerr-Schild only; r_excise <= 0: no excision */
+  int nbx, nby, nbz;                 /* block grid */
+  int nx, ny, nz;                    /* interior zones per block */
+  int ng;                            /* ghosts per side in active dimensions: >=2 for PLM, >=3 for WENO5-Z */
+  double xmin[3], xmax[3];           /* global domain, uniform spacing */
+  int bc[3][2];                      /* [dimension][lower, upper] */
+  double gamma_ad;                   /* ideal gas P = (Gamma-1) rho eps */
+  int recon, riemann, use_ct;
+  double rho_floor, eps_floor, w_max; /* constant-form floors (first case) */
+  double c2p_tol;                     /* relative tolerance on the con2prim root mu */
+  int c2p_maxit;
+} phx_params;
+
+/* Build a mesh object: validates the parameters, allocates flux scratch (3 x one 8-variable field),
+ * the excision flag array and reduction scratch, and runs the geometry-flag kernel on `stream`.
+ * Errors: PHX_EINVAL (bad sizes, ng too small for recon, inactive dimension split over blocks),
+ * PHX_ENOMEM, PHX_ECUDA.  The mesh is freed with phx_free_mesh. */
+int phx_init_mesh(const phx_params* params, void* stream, phx_mesh** out);
+int phx_free_mesh(phx_mesh* mesh);
+
+/* Number of doubles in one 8-variable field: nblocks*8*(nz+2gz)*(ny+2gy)*(nx+2gx). */
+size_t phx_field_elems(const phx_mesh* mesh);
+/* Number of bytes in one mask: phx_field_elems/8. */
+size_t phx_mask_elems(const phx_mesh* mesh);
+
+/* U~ = sqrt(gamma) U(P) (Eq.2) at every allocated cell (ghosts included). */
+int phx_prim_to_cons(const phx_mesh* mesh, const double* d_prim, double* d_cons, void* stream);
+
+/* Primitive recovery after Kastaun et al. 2021 plus floors on every
+ * interior cell, then ghost fill of d_prim.  d_cons is rewritten only where a floor or ceiling acted
+ * (D, S_j, tau recomputed from the floored primitives; B~ untouched).  d_mask receives the per-cell bits. */
+int phx_cons_to_prim(const phx_mesh* mesh, double* d_cons, double* d_prim, unsigned char* d_mask, void* stream);
+
+/* Ghost zones of a primitive field: periodic wrap / zero-gradient outflow at domain faces, copies from the
+ * owning neighbour block elsewhere (faces, edges and corners). */
+int phx_fill_ghosts(const phx_mesh* mesh, double* d_prim, void* stream);
+
+/* One Runge-Kutta stage of Eq.1:  U~ <- g0*U~0 + g1*U~ + beta_dt * [ -div F~ + alpha sqrt(gamma) S ],
+ * with F~ from reconstruction + LLF/HLL + flux-CT, then con2prim, floors and
+ * ghost fill.  RK2 (Heun): (1, 0, dt) then (1/2, 1/2, dt/2).
+ *   in : d_prim = primitives of d_cons with ghosts filled;  d_cons0 = U~ at the start of the step
+ *   out: d_cons updated (interior), d_prim = new primitives with ghosts filled, d_mask = this stage's mask.
+ * d_cons0 may alias d_cons (stage 1). */
+int phx_rk_stage(phx_mesh* mesh, double g0, double g1, double beta_dt, const double* d_cons0, double* d_cons,
+                 double* d_prim, unsigned char* d_mask, void* stream);
+
+/* dt = cfl * min over interior, non-excised cells of 1 / sum_d max(|lambda+^d|, |lambda-^d|)/dx_d.
+ * d_dt (device, required) receives the result; if h_dt is non-NULL the value is also copied to the host
+ * and the stream is synchronised. */
+int phx_cfl_dt(const phx_mesh* mesh, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream);
+
+/* One full RK2 step with the time step read from the device scalar d_dt (no host round trip):
+ * copies U~ to d_cons0, runs both stages; equivalent to two phx_rk_stage calls. */
+int phx_rk2_step(phx_mesh* mesh, const double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
+                 unsigned char* d_mask, void* stream);
+
+/* HOST-buffer path (the end-to-end call): copies h_prim_in (HOST, phx_field_elems doubles, ghosts filled) to
+ * mesh-owned device fields, computes U~ (phx_prim_to_cons), then runs `nsteps` times { phx_cfl_dt ; phx_rk2_step }
+ * with the time step kept on the device, and copies the primitives (required), the conserved variables and the
+ * last stage's mask (both nullable) back to HOST buffers.  *h_t (nullable) receives the elapsed coordinate time.
+ * Synchronises `stream` before returning.  The device workspace (3 fields + mask) is allocated on first use and
+ * freed with the mesh.  Pinned host buffers make the copies asynchronous-capable but are not required. */
+int phx_evolve_host(phx_mesh* mesh, const double* h_prim_in, int nsteps, double cfl, double* h_prim_out,
+                    double* h_cons_out, unsigned char* h_mask_out, double* h_t, void* stream);
+
+/* Face fluxes F~^d (after flux-CT is NOT applied; raw Riemann fluxes) of the last stage, for debugging and tests:
+ * device pointer to the mesh-owned scratch of direction d (0,1,2), layout of one 8-variable field, the
+ * face (i-1/2) stored at cell i. */
+const double* phx_debug_flux(const phx_mesh* mesh, int d);
+
+/* Count of this library's kernel launches since the mesh was created (for bench.py's gpu_launches). */
+unsigned long long phx_launch_count(const phx_mesh* mesh);
+
+const char* phx_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,720 @@
+// phx_kernels.cu — sm_100a kernels and the C ABI of include/phx.h.
+//
+// Kernels per Runge-Kutta stage (all launched on the caller's stream, no host synchronisation):
+//   k_sweep_x      fused reconstruct + Riemann flux along x: one thread per cell, upper-face states exchanged through
+//                  shared memory, flat tiling over (row, i) so that warps stay full for any row length
+//   k_sweep_march  fused reconstruct + Riemann flux along y or z: lanes along x (coalesced), each thread marches along
+//                  the sweep direction with a register window of 2*HW+1 rows, so every primitive is loaded once
+//   k_update       flux-CT + flux divergence + geometric sources + RK combine + con2prim + floors, one thread per cell
+//   k_fill_ghosts  periodic / outflow / block-to-block ghost copies in one gather pass
+// and k_cfl_partial / k_cfl_final (warp-shuffle min reduction), k_prim_to_cons, k_c2p, k_excision_flags.
+#include "phx_device.cuh"
+#include "../../include/phx.h"
+
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+using namespace phx;
+
+// ================================================================================================ kernels
+constexpr int XS_BLOCK = 128;   // threads per block of the x sweep (XS_BLOCK-1 faces per block)
+constexpr int MS_BLOCK = 128;   // threads per block of the marching sweeps
+constexpr int UP_BLOCK = 128;
+
+template <int RECON>
+__device__ __forceinline__ void positivity_fallback(const MeshDev& m, const double* centre, double* qm, double* qp) {
+  if constexpr (RECON == 3) {
+    const double ufl = m.rho_floor * m.eps_floor;
+    if (qm[RHO] <= m.rho_floor || qp[RHO] <= m.rho_floor || qm[UU] <= ufl || qp[UU] <= ufl) {
+#pragma unroll
+      for (int v = 0; v < NV; ++v) { qm[v] = centre[v]; qp[v] = centre[v]; }
+    }
+  }
+}
+
+template <int METRIC, int D>
+__device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G, const double* qL, const double* qR, double* F) {
+  double UL[NV], UR[NV], FL[NV], FR[NV], lmL, lpL, lmR, lpR;
+  state_flux<METRIC, D>(qL, G, m.gam, UL, FL, lmL, lpL);
+  state_flux<METRIC, D>(qR, G, m.gam, UR, FR, lmR, lpR);
+  riemann_combine(m.riemann, UL, UR, FL, FR, lmL, lpL, lmR, lpR, F);
+  F[BX + D] = 0.0;
+}
+
+// ---- x sweep ------------------------------------------------------------------------------------
+// position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
+template <int METRIC, int RECON>
+__global__ void __launch_bounds__(XS_BLOCK) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+                                                      long long npos, int rowlen, int nrj, int nrk, int j0, int k0) {
+  constexpr int HW = ReconTraits<RECON>::HW;
+  __shared__ double sh[NV][XS_BLOCK];
+  const int t = threadIdx.x;
+  const long long p = (long long)blockIdx.x * (XS_BLOCK - 1) + t;
+  const bool valid = p < npos;
+  double qm[NV], qp[NV];
+  long long base = 0;
+  int ii = 0, i = 0, j = 0, k = 0, b = 0;
+  if (valid) {
+    const long long row = p / rowlen;
+    ii = (int)(p - row * rowlen);
+    const int jj = (int)(row % nrj);
+    const long long r2 = row / nrj;
+    const int kk = (int)(r2 % nrk);
+    b = (int)(r2 / nrk);
+    i = m.g[0] - 1 + ii; j = j0 + jj; k = k0 + kk;
+    base = (long long)b * NV * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
+    double centre[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      double f[2 * HW + 1];
+#pragma unroll
+      for (int s = 0; s <= 2 * HW; ++s) f[s] = prim[base + v * m.ncell + (s - HW)];
+      centre[v] = f[HW];
+      recon1<RECON>(f, qm[v], qp[v]);
+    }
+    positivity_fallback<RECON>(m, centre, qm, qp);
+#pragma unroll
+    for (int v = 0; v < NV; ++v) sh[v][t] = qp[v];
+  }
+  __syncthreads();
+  if (!valid || t == 0 || ii == 0) return;
+  double qL[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) qL[v] = sh[v][t - 1];
+  int cb[3];
+  block_coords(m, b, cb);
+  Geo<METRIC> G;
+  G.at(m, xface(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
+  double F[NV];
+  face_flux<METRIC, 0>(m, G, qL, qm, F);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) flux[base + v * m.ncell] = F[v];
+}
+
+// ---- y / z sweep ---------------------------------------------------------------------------------
+// transverse position p -> (t1, t0) with t0 along x (fastest); blockIdx.y = b*nseg + segment.
+template <int METRIC, int RECON, int D>
+__global__ void __launch_bounds__(MS_BLOCK) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+                                                          int ntr, int n0, int lo0, int lo1, int nseg, int L) {
+  constexpr int HW = ReconTraits<RECON>::HW;
+  const int p = blockIdx.x * MS_BLOCK + threadIdx.x;
+  if (p >= ntr) return;
+  const int b = blockIdx.y / nseg;
+  const int seg = blockIdx.y - b * nseg;
+  const int t0 = p % n0, t1 = p / n0;
+  const int i = lo0 + t0;             // x index
+  const int o = lo1 + t1;             // the other transverse index (k for D=1, j for D=2)
+  const long long sd = (D == 1) ? m.sj : m.sk;
+  const long long so = (D == 1) ? m.sk : m.sj;
+  const int f0 = m.g[D] + seg * L;
+  const int f1 = min(f0 + L - 1, m.g[D] + m.n[D]);
+  if (f0 > f1) return;
+  const long long col = (long long)b * NV * m.ncell + (long long)o * so + i;
+  int cb[3];
+  block_coords(m, b, cb);
+  const double xx = xcen(m, 0, cb[0], i);
+  const double xo = (D == 1) ? xcen(m, 2, cb[2], o) : xcen(m, 1, cb[1], o);
+
+  double w[2 * HW + 1][NV];
+#pragma unroll
+  for (int r = 0; r < 2 * HW; ++r)
+#pragma unroll
+    for (int v = 0; v < NV; ++v) w[r][v] = prim[col + v * m.ncell + (long long)(f0 - 1 - HW + r) * sd];
+  double qpPrev[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) qpPrev[v] = 0.0;
+  for (int c = f0 - 1; c <= f1; ++c) {
+#pragma unroll
+    for (int v = 0; v < NV; ++v) w[2 * HW][v] = prim[col + v * m.ncell + (long long)(c + HW) * sd];
+    double qm[NV], qp[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+      double f[2 * HW + 1];
+#pragma unroll
+      for (int s = 0; s <= 2 * HW; ++s) f[s] = w[s][v];
+      recon1<RECON>(f, qm[v], qp[v]);
+    }
+    positivity_fallback<RECON>(m, w[HW], qm, qp);
+    if (c >= f0) {
+      Geo<METRIC> G;
+      const double xf = xface(m, D, cb[D], c);
+      if (D == 1) G.at(m, xx, xf, xo); else G.at(m, xx, xo, xf);
+      double F[NV];
+      face_flux<METRIC, D>(m, G, qpPrev, qm, F);
+#pragma unroll
+      for (int v = 0; v < NV; ++v) flux[col + v * m.ncell + (long long)c * sd] = F[v];
+    }
+#pragma unroll
+    for (int v = 0; v < NV; ++v) qpPrev[v] = qp[v];
+#pragma unroll
+    for (int r = 0; r < 2 * HW; ++r)
+#pragma unroll
+      for (int v = 0; v < NV; ++v) w[r][v] = w[r + 1][v];
+  }
+}
+
+// ---- update: flux-CT + divergence + sources + RK combine + con2prim + floors ----------------------
+struct FluxPtrs { const double* f[3]; };
+
+// contribution of the edge-EMF pair (A, C) (third direction E) to d/dt of B~^C and B~^A, reading C5.3
+template <int A, int C, bool EXC>
+__device__ __forceinline__ void ct_pair(const MeshDev& m, const FluxPtrs& fl, const unsigned char* __restrict__ xfl, long long vb,
+                                        long long fb, long long c, const long long* str, unsigned xbit, double* dB) {
+  const double* FaBc = fl.f[A] + vb + (long long)(BX + C) * m.ncell;
+  const double* FcBa = fl.f[C] + vb + (long long)(BX + A) * m.ncell;
+  auto E = [&](long long id) {
+    double e = 0.25 * (FaBc[id] + FaBc[id - str[C]] - FcBa[id] - FcBa[id - str[A]]);
+    if (EXC) { if (xfl[fb + id] & xbit) e = 0.0; }
+    return e;
+  };
+  const double e00 = E(c), e10 = E(c + str[A]), e01 = E(c + str[C]), e11 = E(c + str[A] + str[C]);
+  dB[C] -= (0.5 * (e10 + e11) - 0.5 * (e00 + e01)) * m.rdx[A];
+  dB[A] -= (-0.5 * (e01 + e11) + 0.5 * (e00 + e10)) * m.rdx[C];
+}
+
+template <int METRIC, bool EXC>
+__global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
+                                                     double bdt_host, const double* __restrict__ d_dt, double beta,
+                                                     const double* cons0, double* cons,
+                                                     double* __restrict__ prim, unsigned char* __restrict__ mask, long long ninterior) {
+  const long long p = (long long)blockIdx.x * UP_BLOCK + threadIdx.x;
+  if (p >= ninterior) return;
+  const int ii = (int)(p % m.n[0]);
+  long long r = p / m.n[0];
+  const int jj = (int)(r % m.n[1]); r /= m.n[1];
+  const int kk = (int)(r % m.n[2]);
+  const int b = (int)(r / m.n[2]);
+  const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
+  const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
+  const long long vb = (long long)b * NV * m.ncell;     // block offset in an 8-variable field
+  const long long fb = (long long)b * m.ncell;          // block offset in a one-variable field
+  if (EXC) {
+    if (xfl[fb + c] & XF_CELL) { mask[fb + c] = M_EXCISED; return; }
+  }
+  const double bdt = d_dt ? beta * (*d_dt) : bdt_host;
+  const long long str[3] = {1, m.sj, m.sk};
+  double R[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) R[v] = 0.0;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    if (!m.act[d]) continue;
+    const double* F = fl.f[d] + vb + c;
+#pragma unroll
+    for (int v = 0; v <= CTAU; ++v) R[v] -= (F[v * m.ncell + str[d]] - F[v * m.ncell]) * m.rdx[d];
+    // magnetic components that flux-CT does not replace (inactive partner direction, or CT switched off)
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc) {
+      if (cc == d) continue;
+      if (m.use_ct && m.act[cc]) continue;
+      R[BX + cc] -= (F[(BX + cc) * m.ncell + str[d]] - F[(BX + cc) * m.ncell]) * m.rdx[d];
+    }
+  }
+  if (m.use_ct) {
+    double dB[3] = {0.0, 0.0, 0.0};
+    if (m.act[0] && m.act[1]) ct_pair<0, 1, EXC>(m, fl, xfl, vb, fb, c, str, XF_E3, dB);
+    if (m.act[1] && m.act[2]) ct_pair<1, 2, EXC>(m, fl, xfl, vb, fb, c, str, XF_E1, dB);
+    if (m.act[2] && m.act[0]) ct_pair<2, 0, EXC>(m, fl, xfl, vb, fb, c, str, XF_E2, dB);
+    R[BX] += dB[0]; R[BY] += dB[1]; R[BZ] += dB[2];
+  }
+  int cb[3];
+  block_coords(m, b, cb);
+  const double x = xcen(m, 0, cb[0], i), y = xcen(m, 1, cb[1], j), z = xcen(m, 2, cb[2], k);
+  if constexpr (METRIC == 1) {
+    double q[NV], S[4];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) q[v] = prim[vb + v * m.ncell + c];
+    ks_sources(m, x, y, z, q, S);
+    R[CS1] += S[0]; R[CS2] += S[1]; R[CS3] += S[2]; R[CTAU] += S[3];
+  }
+  double U[NV], q[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const long long id = vb + v * m.ncell + c;
+    U[v] = g0 * cons0[id] + g1 * cons[id] + bdt * R[v];
+  }
+  Geo<METRIC> G;
+  G.at(m, x, y, z);
+  const unsigned char mk = c2p_cell<METRIC>(m, G, U, q);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    const long long id = vb + v * m.ncell + c;
+    cons[id] = U[v];
+    prim[id] = q[v];
+  }
+  mask[fb + c] = mk;
+}
+
+// ---- stand-alone con2prim, prim->cons ---------------------------------------------------------------
+template <int METRIC, bool EXC>
+__global__ void __launch_bounds__(UP_BLOCK) k_c2p(MeshDev m, const unsigned char* __restrict__ xfl, double* __restrict__ cons,
+                                                  double* __restrict__ prim, unsigned char* __restrict__ mask, long long ninterior) {
+  const long long p = (long long)blockIdx.x * UP_BLOCK + threadIdx.x;
+  if (p >= ninterior) return;
+  const int ii = (int)(p % m.n[0]);
+  long long r = p / m.n[0];
+  const int jj = (int)(r % m.n[1]); r /= m.n[1];
+  const int kk = (int)(r % m.n[2]);
+  const int b = (int)(r / m.n[2]);
+  const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
+  const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
+  const long long vb = (long long)b * NV * m.ncell, fb = (long long)b * m.ncell;
+  if (EXC) {
+    if (xfl[fb + c] & XF_CELL) { mask[fb + c] = M_EXCISED; return; }
+  }
+  int cb[3];
+  block_coords(m, b, cb);
+  Geo<METRIC> G;
+  G.at(m, xcen(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
+  double U[NV], q[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) U[v] = cons[vb + v * m.ncell + c];
+  const unsigned char mk = c2p_cell<METRIC>(m, G, U, q);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) {
+    if (mk & (M_RHO_FLOOR | M_EPS_FLOOR | M_W_CEIL | M_BAD_INPUT)) cons[vb + v * m.ncell + c] = U[v];
+    prim[vb + v * m.ncell + c] = q[v];
+  }
+  mask[fb + c] = mk;
+}
+
+template <int METRIC>
+__global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* __restrict__ prim, double* __restrict__ cons, long long nall) {
+  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (p >= nall) return;
+  const int i = (int)(p % m.na[0]);
+  long long r = p / m.na[0];
+  const int j = (int)(r % m.na[1]); r /= m.na[1];
+  const int k = (int)(r % m.na[2]);
+  const int b = (int)(r / m.na[2]);
+  const long long id = (long long)b * NV * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
+  int cb[3];
+  block_coords(m, b, cb);
+  Geo<METRIC> G;
+  G.at(m, xcen(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
+  double q[NV], U[NV];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) q[v] = prim[id + v * m.ncell];
+  prim_to_cons_pt<METRIC>(q, G, m.gam, U);
+#pragma unroll
+  for (int v = 0; v < NV; ++v) cons[id + v * m.ncell] = U[v];
+}
+
+// ---- ghost fill: one gather pass -------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, long long nall) {
+  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (p >= nall) return;
+  int l[3];
+  l[0] = (int)(p % m.na[0]);
+  long long r = p / m.na[0];
+  l[1] = (int)(r % m.na[1]); r /= m.na[1];
+  l[2] = (int)(r % m.na[2]);
+  const int b = (int)(r / m.na[2]);
+  bool interior = true;
+#pragma unroll
+  for (int d = 0; d < 3; ++d) interior = interior && (l[d] >= m.g[d]) && (l[d] < m.g[d] + m.n[d]);
+  if (interior) return;
+  int cb[3], sb[3], sl[3];
+  block_coords(m, b, cb);
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int gi = cb[d] * m.n[d] + (l[d] - m.g[d]);
+    if (gi < 0) gi = (m.bc[d][0] == 0) ? gi + m.N[d] : 0;
+    else if (gi >= m.N[d]) gi = (m.bc[d][1] == 0) ? gi - m.N[d] : m.N[d] - 1;
+    sb[d] = gi / m.n[d];
+    sl[d] = gi - sb[d] * m.n[d] + m.g[d];
+  }
+  const int bs = (sb[2] * m.nb[1] + sb[1]) * m.nb[0] + sb[0];
+  const long long src = (long long)bs * NV * m.ncell + (long long)sl[2] * m.sk + (long long)sl[1] * m.sj + sl[0];
+  const long long dst = (long long)b * NV * m.ncell + (long long)l[2] * m.sk + (long long)l[1] * m.sj + l[0];
+#pragma unroll
+  for (int v = 0; v < NV; ++v) prim[dst + v * m.ncell] = prim[src + v * m.ncell];
+}
+
+// ---- CFL: warp-shuffle min reduction ------------------------------------------------------------------
+template <int METRIC, bool EXC>
+__global__ void __launch_bounds__(256) k_cfl_partial(MeshDev m, const unsigned char* __restrict__ xfl, const double* __restrict__ prim,
+                                                     double* __restrict__ partial, long long ninterior) {
+  double best = INFINITY;
+  for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < ninterior; p += (long long)gridDim.x * 256) {
+    const int ii = (int)(p % m.n[0]);
+    long long r = p / m.n[0];
+    const int jj = (int)(r % m.n[1]); r /= m.n[1];
+    const int kk = (int)(r % m.n[2]);
+    const int b = (int)(r / m.n[2]);
+    const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
+    const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
+    if (EXC) { if (xfl[(long long)b * m.ncell + c] & XF_CELL) continue; }
+    int cb[3];
+    block_coords(m, b, cb);
+    Geo<METRIC> G;
+    G.at(m, xcen(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
+    double q[NV], lam[3];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) q[v] = prim[(long long)b * NV * m.ncell + v * m.ncell + c];
+    max_speeds<METRIC>(q, G, m.gam, lam);
+    double s = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) if (m.act[d]) s += lam[d] * m.rdx[d];
+    best = fmin(best, 1.0 / s);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  __shared__ double sh[8];
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double v = (threadIdx.x < 8) ? sh[threadIdx.x] : INFINITY;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (threadIdx.x == 0) partial[blockIdx.x] = v;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_cfl_final(const double* __restrict__ partial, int n, double cfl, double* __restrict__ dt) {
+  double best = INFINITY;
+  for (int p = threadIdx.x; p < n; p += 256) best = fmin(best, partial[p]);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  __shared__ double sh[8];
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    double v = (threadIdx.x < 8) ? sh[threadIdx.x] : INFINITY;
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (threadIdx.x == 0) *dt = cfl * v;
+  }
+}
+
+// ---- excision flags (init only) ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_excision_flags(MeshDev m, unsigned char* __restrict__ xfl, long long nall) {
+  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
+  if (p >= nall) return;
+  int l[3];
+  l[0] = (int)(p % m.na[0]);
+  long long r = p / m.na[0];
+  l[1] = (int)(r % m.na[1]); r /= m.na[1];
+  l[2] = (int)(r % m.na[2]);
+  const int b = (int)(r / m.na[2]);
+  int cb[3];
+  block_coords(m, b, cb);
+  auto ex = [&](int di, int dj, int dk) {
+    double rr, H, lv[3];
+    ks_scalars(m, xcen(m, 0, cb[0], l[0] - di), xcen(m, 1, cb[1], l[1] - dj), xcen(m, 2, cb[2], l[2] - dk), rr, H, lv);
+    return rr < m.r_exc;
+  };
+  unsigned f = 0;
+  if (ex(0, 0, 0)) f |= XF_CELL;
+  if (ex(0, 0, 0) || ex(0, 1, 0) || ex(0, 0, 1) || ex(0, 1, 1)) f |= XF_E1;   // edge (j-1/2, k-1/2)
+  if (ex(0, 0, 0) || ex(1, 0, 0) || ex(0, 0, 1) || ex(1, 0, 1)) f |= XF_E2;   // edge (i-1/2, k-1/2)
+  if (ex(0, 0, 0) || ex(1, 0, 0) || ex(0, 1, 0) || ex(1, 1, 0)) f |= XF_E3;   // edge (i-1/2, j-1/2)
+  xfl[p] = (unsigned char)f;
+}
+
+// ================================================================================================ host side
+struct phx_mesh {
+  MeshDev m;
+  phx_params par;
+  double* flux[3];
+  unsigned char* xfl;
+  double* partial;
+  int npartial;
+  unsigned long long launches;
+  long long nall, ninterior;
+  // workspace of the host-buffer path (phx_evolve_host), allocated on first use
+  double* ws_field[3];
+  unsigned char* ws_mask;
+  double* ws_scal;   // [0] dt, [1] t
+};
+
+static thread_local char g_err[512] = "";
+static int fail(int code, const char* msg) {
+  snprintf(g_err, sizeof g_err, "%s", msg);
+  return code;
+}
+static int cuda_fail(cudaError_t e, const char* where) {
+  snprintf(g_err, sizeof g_err, "%s: %s", where, cudaGetErrorString(e));
+  return PHX_ECUDA;
+}
+#define CUDA_TRY(x, where) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+#define LAUNCH_CHECK(mesh, where) do { (mesh)->launches++; cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_, where); } while (0)
+
+static bool aligned16(const void* p) { return p && (((uintptr_t)p) & 15u) == 0; }
+
+extern "C" const char* phx_last_error(void) { return g_err; }
+
+extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) {
+  if (!p || !out) return fail(PHX_EINVAL, "phx_init_mesh: null argument");
+  *out = nullptr;
+  if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->nbx < 1 || p->nby < 1 || p->nbz < 1) return fail(PHX_EINVAL, "phx_init_mesh: sizes must be >= 1");
+  if (p->metric != PHX_MINKOWSKI && p->metric != PHX_KERR_SCHILD) return fail(PHX_EINVAL, "phx_init_mesh: unknown metric");
+  if (p->recon < 0 || p->recon > 3) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown reconstruction");
+  if (p->riemann < 0 || p->riemann > 1) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown Riemann solver");
+  const int need = (p->recon == 3) ? 3 : 2;
+  if (p->ng < need) return fail(PHX_EINVAL, "phx_init_mesh: ng too small for the reconstruction stencil (>=2 PLM, >=3 WENO5-Z)");
+  if (!(p->gamma_ad > 1.0)) return fail(PHX_EINVAL, "phx_init_mesh: gamma_ad must exceed 1");
+  if (!(p->rho_floor > 0.0) || !(p->eps_floor > 0.0) || !(p->w_max > 1.0)) return fail(PHX_EINVAL, "phx_init_mesh: floors must be positive, w_max > 1");
+  if (!(p->c2p_tol > 0.0) || p->c2p_maxit < 1) return fail(PHX_EINVAL, "phx_init_mesh: c2p_tol > 0 and c2p_maxit >= 1 required");
+  if (p->metric == PHX_KERR_SCHILD && !(p->bh_mass > 0.0)) return fail(PHX_EINVAL, "phx_init_mesh: bh_mass must be positive");
+  phx_mesh* M = new (std::nothrow) phx_mesh();
+  if (!M) return fail(PHX_ENOMEM, "phx_init_mesh: host allocation failed");
+  memset(M, 0, sizeof *M);
+  M->par = *p;
+  MeshDev& m = M->m;
+  m.metric = p->metric; m.M = p->bh_mass; m.a = p->bh_spin; m.r_exc = p->r_excise;
+  m.nb[0] = p->nbx; m.nb[1] = p->nby; m.nb[2] = p->nbz;
+  m.n[0] = p->nx; m.n[1] = p->ny; m.n[2] = p->nz;
+  for (int d = 0; d < 3; ++d) {
+    m.N[d] = m.nb[d] * m.n[d];
+    m.act[d] = m.N[d] > 1;
+    if (!m.act[d]) { /* nothing */ }
+    if (m.act[d] && m.n[d] < p->ng) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: an active dimension needs at least ng zones per block"); }
+    m.g[d] = m.act[d] ? p->ng : 0;
+    m.na[d] = m.n[d] + 2 * m.g[d];
+    if (!(p->xmax[d] > p->xmin[d])) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: xmax must exceed xmin"); }
+    m.xmin[d] = p->xmin[d];
+    m.dx[d] = (p->xmax[d] - p->xmin[d]) / m.N[d];
+    m.rdx[d] = 1.0 / m.dx[d];
+    for (int s = 0; s < 2; ++s) {
+      if (p->bc[d][s] != PHX_BC_PERIODIC && p->bc[d][s] != PHX_BC_OUTFLOW) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: unknown boundary condition"); }
+      m.bc[d][s] = p->bc[d][s];
+    }
+  }
+  m.nblk = m.nb[0] * m.nb[1] * m.nb[2];
+  m.sj = m.na[0];
+  m.sk = (long long)m.na[0] * m.na[1];
+  m.ncell = m.sk * m.na[2];
+  m.gam = p->gamma_ad; m.recon = p->recon; m.riemann = p->riemann; m.use_ct = p->use_ct ? 1 : 0;
+  m.rho_floor = p->rho_floor; m.eps_floor = p->eps_floor; m.w_max = p->w_max; m.c2p_tol = p->c2p_tol; m.c2p_maxit = p->c2p_maxit;
+  m.excise = (p->metric == PHX_KERR_SCHILD && p->r_excise > 0.0) ? 1 : 0;
+  M->nall = (long long)m.nblk * m.ncell;
+  M->ninterior = (long long)m.nblk * m.n[0] * m.n[1] * m.n[2];
+  if (M->nall * NV >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
+  const size_t fbytes = (size_t)M->nall * NV * sizeof(double);
+  cudaStream_t st = (cudaStream_t)stream;
+  for (int d = 0; d < 3; ++d) {
+    if (!m.act[d]) continue;
+    cudaError_t e = cudaMalloc((void**)&M->flux[d], fbytes);
+    if (e != cudaSuccess) { phx_free_mesh(M); return (e == cudaErrorMemoryAllocation) ? fail(PHX_ENOMEM, "phx_init_mesh: out of device memory (flux scratch)") : cuda_fail(e, "cudaMalloc"); }
+    e = cudaMemsetAsync(M->flux[d], 0, fbytes, st);
+    if (e != cudaSuccess) { phx_free_mesh(M); return cuda_fail(e, "cudaMemsetAsync"); }
+  }
+  M->npartial = 148 * 8;
+  if (cudaMalloc((void**)&M->partial, sizeof(double) * M->npartial) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
+  if (m.excise) {
+    if (cudaMalloc((void**)&M->xfl, (size_t)M->nall) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
+    k_excision_flags<<<(unsigned)((M->nall + 255) / 256), 256, 0, st>>>(m, M->xfl, M->nall);
+    M->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { phx_free_mesh(M); return cuda_fail(e, "k_excision_flags"); }
+  }
+  *out = M;
+  return PHX_OK;
+}
+
+extern "C" int phx_free_mesh(phx_mesh* M) {
+  if (!M) return PHX_OK;
+  for (int d = 0; d < 3; ++d) if (M->flux[d]) cudaFree(M->flux[d]);
+  if (M->xfl) cudaFree(M->xfl);
+  if (M->partial) cudaFree(M->partial);
+  for (int d = 0; d < 3; ++d) if (M->ws_field[d]) cudaFree(M->ws_field[d]);
+  if (M->ws_mask) cudaFree(M->ws_mask);
+  if (M->ws_scal) cudaFree(M->ws_scal);
+  delete M;
+  return PHX_OK;
+}
+
+extern "C" size_t phx_field_elems(const phx_mesh* M) { return M ? (size_t)M->nall * NV : 0; }
+extern "C" size_t phx_mask_elems(const phx_mesh* M) { return M ? (size_t)M->nall : 0; }
+extern "C" unsigned long long phx_launch_count(const phx_mesh* M) { return M ? M->launches : 0; }
+extern "C" const double* phx_debug_flux(const phx_mesh* M, int d) { return (M && d >= 0 && d < 3) ? M->flux[d] : nullptr; }
+
+#define DISPATCH_METRIC(mesh, CALL)                 \
+  do {                                              \
+    if ((mesh)->m.metric == 0) { CALL(0); }         \
+    else { CALL(1); }                               \
+  } while (0)
+
+extern "C" int phx_prim_to_cons(const phx_mesh* Mc, const double* d_prim, double* d_cons, void* stream) {
+  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+  if (!M || !aligned16(d_prim) || !aligned16(d_cons)) return fail(PHX_EINVAL, "phx_prim_to_cons: null or misaligned argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  const unsigned nb = (unsigned)((M->nall + 255) / 256);
+#define CALL(MET) k_prim_to_cons<MET><<<nb, 256, 0, st>>>(M->m, d_prim, d_cons, M->nall)
+  DISPATCH_METRIC(M, CALL);
+#undef CALL
+  LAUNCH_CHECK(M, "k_prim_to_cons");
+  return PHX_OK;
+}
+
+extern "C" int phx_fill_ghosts(const phx_mesh* Mc, double* d_prim, void* stream) {
+  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+  if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
+  if (M->nall == M->ninterior) return PHX_OK;
+  k_fill_ghosts<<<(unsigned)((M->nall + 255) / 256), 256, 0, (cudaStream_t)stream>>>(M->m, d_prim, M->nall);
+  LAUNCH_CHECK(M, "k_fill_ghosts");
+  return PHX_OK;
+}
+
+extern "C" int phx_cons_to_prim(const phx_mesh* Mc, double* d_cons, double* d_prim, unsigned char* d_mask, void* stream) {
+  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+  if (!M || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask) return fail(PHX_EINVAL, "phx_cons_to_prim: null or misaligned argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
+#define CALL(MET)                                                                                         \
+  if (M->m.excise) k_c2p<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior); \
+  else k_c2p<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior)
+  DISPATCH_METRIC(M, CALL);
+#undef CALL
+  LAUNCH_CHECK(M, "k_c2p");
+  return phx_fill_ghosts(M, d_prim, stream);
+}
+
+// ---- sweeps -------------------------------------------------------------------------------------------------
+template <int METRIC, int RECON>
+static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
+  const MeshDev& m = M->m;
+  int lo[3], cnt[3];
+  for (int d = 0; d < 3; ++d) {
+    lo[d] = m.act[d] ? m.g[d] - 1 : 0;
+    cnt[d] = m.act[d] ? m.n[d] + 2 : 1;
+  }
+  if (m.act[0]) {
+    const int rowlen = m.n[0] + 2;
+    const long long npos = (long long)m.nblk * cnt[2] * cnt[1] * rowlen;
+    const unsigned nb = (unsigned)((npos + (XS_BLOCK - 2)) / (XS_BLOCK - 1));
+    k_sweep_x<METRIC, RECON><<<nb, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], npos, rowlen, cnt[1], cnt[2], lo[1], lo[2]);
+    M->launches++;
+  }
+  const int Lmax = 33;
+  if (m.act[1]) {
+    const int nfaces = m.n[1] + 1;
+    const int nseg = (nfaces + Lmax - 1) / Lmax;
+    const int L = (nfaces + nseg - 1) / nseg;
+    const int ntr = cnt[0] * cnt[2];
+    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, m.nblk * nseg);
+    k_sweep_march<METRIC, RECON, 1><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], nseg, L);
+    M->launches++;
+  }
+  if (m.act[2]) {
+    const int nfaces = m.n[2] + 1;
+    const int nseg = (nfaces + Lmax - 1) / Lmax;
+    const int L = (nfaces + nseg - 1) / nseg;
+    const int ntr = cnt[0] * cnt[1];
+    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, m.nblk * nseg);
+    k_sweep_march<METRIC, RECON, 2><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], nseg, L);
+    M->launches++;
+  }
+}
+
+static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
+  const int key = M->m.metric * 4 + M->m.recon;
+  switch (key) {
+    case 0: launch_sweeps_t<0, 0>(M, prim, st); break;
+    case 1: launch_sweeps_t<0, 1>(M, prim, st); break;
+    case 2: launch_sweeps_t<0, 2>(M, prim, st); break;
+    case 3: launch_sweeps_t<0, 3>(M, prim, st); break;
+    case 4: launch_sweeps_t<1, 0>(M, prim, st); break;
+    case 5: launch_sweeps_t<1, 1>(M, prim, st); break;
+    case 6: launch_sweeps_t<1, 2>(M, prim, st); break;
+    default: launch_sweeps_t<1, 3>(M, prim, st); break;
+  }
+}
+
+static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
+                      double* d_cons, double* d_prim, unsigned char* d_mask, cudaStream_t st) {
+  launch_sweeps(M, d_prim, st);
+  { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
+  FluxPtrs fl;
+  for (int d = 0; d < 3; ++d) fl.f[d] = M->flux[d];
+  const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
+#define CALL(MET)                                                                                                                   \
+  if (M->m.excise) k_update<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons, d_prim, d_mask, M->ninterior); \
+  else k_update<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons, d_prim, d_mask, M->ninterior)
+  DISPATCH_METRIC(M, CALL);
+#undef CALL
+  LAUNCH_CHECK(M, "k_update");
+  return phx_fill_ghosts(M, d_prim, st);
+}
+
+extern "C" int phx_rk_stage(phx_mesh* M, double g0, double g1, double beta_dt, const double* d_cons0, double* d_cons, double* d_prim,
+                            unsigned char* d_mask, void* stream) {
+  if (!M || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask)
+    return fail(PHX_EINVAL, "phx_rk_stage: null or misaligned argument");
+  return stage_impl(M, g0, g1, beta_dt, nullptr, 0.0, d_cons0, d_cons, d_prim, d_mask, (cudaStream_t)stream);
+}
+
+extern "C" int phx_rk2_step(phx_mesh* M, const double* d_dt, double* d_cons0, double* d_cons, double* d_prim, unsigned char* d_mask,
+                            void* stream) {
+  if (!M || !d_dt || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask || d_cons0 == d_cons)
+    return fail(PHX_EINVAL, "phx_rk2_step: null, misaligned or aliased argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  // U~0 <- U~, then both stages in place on d_cons
+  CUDA_TRY(cudaMemcpyAsync(d_cons0, d_cons, (size_t)M->nall * NV * sizeof(double), cudaMemcpyDeviceToDevice, st), "cudaMemcpyAsync");
+  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons0, d_cons, d_prim, d_mask, st);
+  if (rc != PHX_OK) return rc;
+  return stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons0, d_cons, d_prim, d_mask, st);
+}
+
+extern "C" int phx_cfl_dt(const phx_mesh* Mc, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream) {
+  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+  if (!M || !aligned16(d_prim) || !d_dt || !(cfl > 0.0)) return fail(PHX_EINVAL, "phx_cfl_dt: null or misaligned argument, or cfl <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  long long want = (M->ninterior + 255) / 256;
+  const int nb = (int)(want < M->npartial ? want : M->npartial);
+#define CALL(MET)                                                                                          \
+  if (M->m.excise) k_cfl_partial<MET, true><<<nb, 256, 0, st>>>(M->m, M->xfl, d_prim, M->partial, M->ninterior); \
+  else k_cfl_partial<MET, false><<<nb, 256, 0, st>>>(M->m, M->xfl, d_prim, M->partial, M->ninterior)
+  DISPATCH_METRIC(M, CALL);
+#undef CALL
+  LAUNCH_CHECK(M, "k_cfl_partial");
+  k_cfl_final<<<1, 256, 0, st>>>(M->partial, nb, cfl, d_dt);
+  LAUNCH_CHECK(M, "k_cfl_final");
+  if (h_dt) {
+    CUDA_TRY(cudaMemcpyAsync(h_dt, d_dt, sizeof(double), cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
+    CUDA_TRY(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  }
+  return PHX_OK;
+}
+
+// ---- host-buffer path ------------------------------------------------------------------------------------------
+__global__ void k_accumulate_time(double* __restrict__ scal) { scal[1] += scal[0]; }
+
+extern "C" int phx_evolve_host(phx_mesh* M, const double* h_prim_in, int nsteps, double cfl, double* h_prim_out, double* h_cons_out,
+                               unsigned char* h_mask_out, double* h_t, void* stream) {
+  if (!M || !h_prim_in || !h_prim_out || nsteps < 0 || !(cfl > 0.0)) return fail(PHX_EINVAL, "phx_evolve_host: null argument, nsteps < 0 or cfl <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t fbytes = (size_t)M->nall * NV * sizeof(double);
+  if (!M->ws_scal) {
+    for (int d = 0; d < 3; ++d)
+      if (cudaMalloc((void**)&M->ws_field[d], fbytes) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
+    if (cudaMalloc((void**)&M->ws_mask, (size_t)M->nall) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
+    if (cudaMalloc((void**)&M->ws_scal, 2 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
+  }
+  double* prim = M->ws_field[0];
+  double* cons = M->ws_field[1];
+  double* cons0 = M->ws_field[2];
+  CUDA_TRY(cudaMemcpyAsync(prim, h_prim_in, fbytes, cudaMemcpyHostToDevice, st), "cudaMemcpyAsync H2D");
+  CUDA_TRY(cudaMemsetAsync(M->ws_scal, 0, 2 * sizeof(double), st), "cudaMemsetAsync");
+  CUDA_TRY(cudaMemsetAsync(M->ws_mask, 0, (size_t)M->nall, st), "cudaMemsetAsync");
+  int rc = phx_prim_to_cons(M, prim, cons, st);
+  if (rc != PHX_OK) return rc;
+  for (int s = 0; s < nsteps; ++s) {
+    rc = phx_cfl_dt(M, prim, cfl, M->ws_scal, nullptr, st);
+    if (rc != PHX_OK) return rc;
+    rc = phx_rk2_step(M, M->ws_scal, cons0, cons, prim, M->ws_mask, st);
+    if (rc != PHX_OK) return rc;
+    k_accumulate_time<<<1, 1, 0, st>>>(M->ws_scal);
+    LAUNCH_CHECK(M, "k_accumulate_time");
+  }
+  CUDA_TRY(cudaMemcpyAsync(h_prim_out, prim, fbytes, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
+  if (h_cons_out) CUDA_TRY(cudaMemcpyAsync(h_cons_out, cons, fbytes, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
+  if (h_mask_out) CUDA_TRY(cudaMemcpyAsync(h_mask_out, M->ws_mask, (size_t)M->nall, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
+  double scal[2] = {0.0, 0.0};
+  CUDA_TRY(cudaMemcpyAsync(scal, M->ws_scal, sizeof scal, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
+  CUDA_TRY(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  if (h_t) *h_t = scal[1];
+  return PHX_OK;
+}

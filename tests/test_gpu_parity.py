@@ -1,0 +1,314 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are BASELINE.json's: <= 1e-11 relative per conserved variable after one RK2 step,
+<= 1e-8 after 100 steps, identical con2prim / floor masks.  Every test here needs a B200 (`-m gpu`).
+"""
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2410_09146_b200 import workloads as wl
+
+from harness import (GpuRun, MARGIN_MIN, TOL_100STEP, TOL_1STEP, compare, interior, run_both, var_errors)
+
+pytestmark = pytest.mark.gpu
+
+
+def _gpu():
+    import torch
+    from paper_2410_09146_b200 import phx
+    assert torch.cuda.is_available(), "these tests must run on the GPU box"
+    return torch, phx
+
+
+def small_workloads():
+    """Sizes the oracle finishes in seconds that still span several thread blocks and ragged tails."""
+    out = {}
+    out["cfg1_shock_tube_256"] = wl.shock_tube(256)
+    out["cfg2_box_24_mc_llf"] = wl.periodic_box(24)
+    out["cfg2_box_20_minmod_hll"] = wl.periodic_box(20, recon=wl.RECON_PLM_MINMOD, riemann=wl.RIEMANN_HLL)
+    out["cfg2_box_12_const_llf"] = wl.periodic_box(12, recon=wl.RECON_CONST)
+    out["cfg3_ks_torus_28"] = wl.kerr_schild_torus(28)
+    out["cfg4_turb_24_weno"] = wl.turbulence_box(24)
+    out["cfg5_blocks_2x2x2_of_12"] = wl.packed_blocks((2, 2, 2), 12)
+    out["cfg5_blocks_3x2x1_of_8"] = wl.packed_blocks((3, 2, 1), 8)
+    return out
+
+
+WORKLOADS = small_workloads()
+
+
+# ----------------------------------------------------------------------------- point-wise ops
+@pytest.mark.parametrize("name", ["cfg2_box_24_mc_llf", "cfg3_ks_torus_28", "cfg5_blocks_2x2x2_of_12", "cfg1_shock_tube_256"])
+def test_prim_to_cons_matches_oracle(name):
+    torch, phx = _gpu()
+    w = WORKLOADS[name]
+    p = w["params"]
+    ref = orc.prim_to_cons(p, w["prim"])
+    mesh = phx.init_mesh(p)
+    prim = torch.from_numpy(w["prim"]).cuda()
+    cons = torch.empty_like(prim)
+    phx.prim_to_cons(mesh, prim, cons)
+    got = cons.cpu().numpy()
+    # every allocated cell (ghosts included), 1e-13 relative to the variable's scale
+    for v in range(8):
+        scale = np.abs(ref[:, v]).max() or 1.0
+        assert np.abs(got[:, v] - ref[:, v]).max() / scale < 1e-13, v
+
+
+@pytest.mark.parametrize("name", ["cfg2_box_24_mc_llf", "cfg3_ks_torus_28", "cfg4_turb_24_weno", "cfg5_blocks_2x2x2_of_12"])
+def test_cons_to_prim_matches_oracle(name):
+    torch, phx = _gpu()
+    w = WORKLOADS[name]
+    p = w["params"]
+    cons_in = orc.prim_to_cons(p, w["prim"])
+    orc.reset_c2p_margin()
+    cons_ref = cons_in.copy()
+    prim_ref, mask_ref = orc.cons_to_prim(p, cons_ref)
+    assert orc.last_c2p_margin() > MARGIN_MIN
+    mesh = phx.init_mesh(p)
+    cons = torch.from_numpy(cons_in).cuda()
+    prim = torch.zeros_like(cons)
+    mask = torch.zeros(mask_ref.shape, dtype=torch.uint8, device="cuda")
+    phx.cons_to_prim(mesh, cons, prim, mask)
+    assert np.array_equal(interior(p, mask.cpu().numpy()), interior(p, mask_ref))
+    got = interior(p, prim.cpu().numpy()); ref = interior(p, prim_ref)
+    ex = interior(p, mask_ref) & 64
+    for v in range(8):
+        scale = np.abs(ref[v]).max() or 1.0
+        e = np.abs(got[v] - ref[v])[ex == 0].max() / scale
+        assert e < 1e-12, (v, e)
+    # ghosts are filled by the call
+    pg = prim.cpu().numpy()
+    assert np.abs(pg - prim_ref).max() <= 1e-12 * np.abs(prim_ref).max()
+
+
+def test_cons_to_prim_floors_and_failure_masks():
+    """Random conserved states that hit every mask bit: density / energy floors, Lorentz ceiling, clipped
+    energy, bad input.  Masks must be identical, floored cells re-densitised identically."""
+    torch, phx = _gpu()
+    n = 16
+    p = wl.default_params(nx=n, ny=n, nz=n, ng=2, rho_floor=1e-3, eps_floor=1e-2, w_max=5.0)
+    rng = np.random.default_rng(wl.SEED0 + 77)
+    for attempt in range(5):
+        q = np.zeros((8, n, n, n))
+        q[0] = 10 ** rng.uniform(-5, 1, (n, n, n))
+        q[1:4] = rng.uniform(-1, 1, (3, n, n, n)) * 10 ** rng.uniform(-2, 1.2, (n, n, n))
+        q[4] = q[0] * 10 ** rng.uniform(-4, 1, (n, n, n))
+        q[5:8] = rng.uniform(-1, 1, (3, n, n, n))
+        prim = wl.finish(p, q)
+        cons_in = orc.prim_to_cons(p, prim)
+        g = 2
+        cons_in[0, 0, g + 1, g + 1, g + 1] = -1.0          # D <= 0
+        cons_in[0, 4, g + 2, g + 2, g + 2] = np.nan        # non-finite tau
+        cons_in[0, 4, g + 3, g + 3, g: g + n] = -0.3 * cons_in[0, 0, g + 3, g + 3, g: g + n]   # tau < 0: clipped energy
+        orc.reset_c2p_margin()
+        cons_ref = cons_in.copy()
+        prim_ref, mask_ref = orc.cons_to_prim(p, cons_ref)
+        if orc.last_c2p_margin() > MARGIN_MIN:
+            break
+    else:
+        pytest.fail("no seed with a safe margin found")
+    bits = np.bitwise_or.reduce(interior(p, mask_ref).ravel())
+    assert bits & 1 and bits & 2 and bits & 4 and bits & 8 and bits & 32, bits
+    mesh = phx.init_mesh(p)
+    cons = torch.from_numpy(cons_in).cuda()
+    prim_g = torch.zeros_like(cons)
+    mask = torch.zeros(mask_ref.shape, dtype=torch.uint8, device="cuda")
+    phx.cons_to_prim(mesh, cons, prim_g, mask)
+    mg = interior(p, mask.cpu().numpy()); mr = interior(p, mask_ref)
+    assert np.array_equal(mg, mr), np.argwhere(mg != mr)[:10]
+    got = interior(p, prim_g.cpu().numpy()); ref = interior(p, prim_ref)
+    # point-wise relative comparison (states span many decades)
+    den = np.maximum(np.abs(ref), 1e-3 * np.abs(ref).max(axis=0, keepdims=True) + 1e-300)
+    assert (np.abs(got - ref) / den).max() < 1e-9
+    cg = interior(p, cons.cpu().numpy()); cr = interior(p, cons_ref)
+    fin = np.isfinite(cr)
+    assert np.array_equal(np.isfinite(cg), fin)
+    denc = np.maximum(np.abs(cr[fin]), 1e-300)
+    floored = (mr & (1 | 2 | 8 | 32)) != 0
+    assert (np.abs(cg - cr)[fin] / denc).max() < 1e-9
+    # untouched where no floor acted: bitwise
+    keep = np.broadcast_to(~floored, cg.shape) & fin
+    assert np.array_equal(cg[keep], interior(p, cons_in)[keep])
+
+
+@pytest.mark.parametrize("name", ["cfg2_box_24_mc_llf", "cfg5_blocks_3x2x1_of_8", "cfg1_shock_tube_256"])
+def test_fill_ghosts_bit_exact(name):
+    torch, phx = _gpu()
+    w = WORKLOADS[name]
+    p = w["params"]
+    rng = np.random.default_rng(5)
+    prim = rng.standard_normal(w["prim"].shape)
+    ref = orc.fill_ghosts(p, prim.copy())
+    mesh = phx.init_mesh(p)
+    t = torch.from_numpy(prim).cuda()
+    phx.fill_ghosts(mesh, t)
+    assert np.array_equal(t.cpu().numpy(), ref)
+
+
+@pytest.mark.parametrize("name", list(WORKLOADS))
+def test_cfl_dt_matches_oracle(name):
+    torch, phx = _gpu()
+    w = WORKLOADS[name]
+    p = w["params"]
+    ref = orc.cfl_dt(p, w["prim"], 0.4)
+    g = GpuRun(p, w["prim"])
+    got = g.dt(0.4)
+    assert abs(got - ref) <= 1e-13 * ref
+    assert abs(float(g.d_dt.cpu()) - got) == 0.0
+
+
+# ----------------------------------------------------------------------------- the RK2 step
+@pytest.mark.parametrize("name", list(WORKLOADS))
+def test_one_rk2_step_matches_oracle(name):
+    w = WORKLOADS[name]
+    p = w["params"]
+    o, g = run_both(p, w["prim"], nsteps=1, cfl=w["cfl"])
+    err = compare(p, o, g, TOL_1STEP)
+    print(name, "1-step err per variable", err)
+
+
+@pytest.mark.parametrize("name", ["cfg2_box_24_mc_llf", "cfg4_turb_24_weno"])
+def test_raw_riemann_fluxes_match_oracle_without_ct(name):
+    """Face fluxes of one stage (CT off so that the oracle's hook returns the raw Riemann fluxes)."""
+    torch, phx = _gpu()
+    w = WORKLOADS[name]
+    p = dict(w["params"]); p["use_ct"] = 0
+    F = orc.stage_fluxes(p, w["prim"])
+    # a zero-dt stage leaves the state alone and the raw fluxes in the mesh-owned scratch
+    g2 = GpuRun(p, w["prim"])
+    phx.rk_stage(g2.mesh, 1.0, 0.0, 0.0, g2.cons, g2.cons, g2.prim, g2.mask)
+    gx, gy, gz = wl.ghosts(p)
+    nx, ny, nz = p["nx"], p["ny"], p["nz"]
+    for d in range(3):
+        got = g2.mesh.debug_flux(d, w["prim"].shape).cpu().numpy()
+        sl = [slice(gz, gz + nz), slice(gy, gy + ny), slice(gx, gx + nx)]
+        sl[2 - d] = slice(sl[2 - d].start, sl[2 - d].stop + 1)
+        a = got[(slice(None), slice(None)) + tuple(sl)]; b = F[d][(slice(None), slice(None)) + tuple(sl)]
+        for v in range(8):
+            scale = np.abs(b[:, v]).max() or 1.0
+            assert np.abs(a[:, v] - b[:, v]).max() / scale < 1e-13, (d, v)
+
+
+def test_shock_tube_to_t_end_matches_oracle():
+    """Config 1 in full: 256 zones to t = 0.4 (about 250 steps) within the 100-step tolerance."""
+    w = WORKLOADS["cfg1_shock_tube_256"]
+    p = w["params"]
+    o, g = run_both(p, w["prim"], cfl=0.4, t_end=0.4)
+    assert 200 < len(o.dts) < 320
+    err = compare(p, o, g, TOL_100STEP)
+    # B^x is bitwise constant in 1-D on both sides
+    assert np.all(interior(p, g.get()[1])[5] == 0.5)
+    print("shock tube", len(o.dts), "steps, err", err)
+
+
+@pytest.mark.parametrize("name,nsteps", [("cfg2_box_24_mc_llf", 100), ("cfg4_turb_24_weno", 20), ("cfg3_ks_torus_28", 50),
+                                         ("cfg5_blocks_2x2x2_of_12", 20)])
+def test_many_steps_match_oracle(name, nsteps):
+    w = WORKLOADS[name]
+    p = w["params"]
+    o, g = run_both(p, w["prim"], nsteps=nsteps, cfl=w["cfl"])
+    err = compare(p, o, g, TOL_100STEP)
+    print(name, nsteps, "steps, err", err)
+
+
+def test_device_dt_step_equals_host_dt_step():
+    """phx_cfl_dt + phx_rk2_step (dt on the device, the configuration bench.py times) gives bitwise the same
+    state as two phx_rk_stage calls with the same dt passed from the host."""
+    w = WORKLOADS["cfg4_turb_24_weno"]
+    p = w["params"]
+    a = GpuRun(p, w["prim"]); b = GpuRun(p, w["prim"])
+    for _ in range(3):
+        dt = a.dt(0.4)
+        a.step(dt)
+        b.step_device_dt(0.4)
+    ca, pa, _, ma = a.get(); cb, pb, _, mb = b.get()
+    assert np.array_equal(ca, cb) and np.array_equal(pa, pb) and np.array_equal(ma, mb)
+
+
+# ----------------------------------------------------------------------------- exact properties on the GPU
+@pytest.mark.parametrize("recon", [0, 1, 2, 3])
+@pytest.mark.parametrize("riemann", [0, 1])
+def test_uniform_state_stays_bitwise_uniform_on_gpu(recon, riemann):
+    n = 20
+    p = wl.default_params(nx=n, ny=n, nz=n, ng=4, recon=recon, riemann=riemann)
+    q = np.zeros((8, n, n, n))
+    q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7] = 1.3, 0.4, -0.2, 0.1, 2.1, 0.7, -0.3, 0.2
+    g = GpuRun(p, wl.finish(p, q))
+    c0 = g.cons.cpu().numpy().copy()
+    for _ in range(3):
+        g.step(g.dt(0.4))
+    cons = g.get()[0]
+    assert np.array_equal(interior(p, cons), interior(p, c0))
+
+
+def test_block_decomposition_is_bitwise_invariant_on_gpu():
+    w = wl.packed_blocks((1, 1, 1), 24)
+    p1 = w["params"]
+    p8, prim8 = wl.reblock(p1, w["prim"], (2, 3, 2))
+    a = GpuRun(p1, w["prim"]); b = GpuRun(p8, prim8)
+    for _ in range(3):
+        dt = a.dt(0.4)
+        assert b.dt(0.4) == dt
+        a.step(dt); b.step(dt)
+    ca, pa, _, ma = a.get(); cb, pb, _, mb = b.get()
+    assert np.array_equal(interior(p1, ca), interior(p8, cb))
+    assert np.array_equal(interior(p1, pa), interior(p8, pb))
+    assert np.array_equal(interior(p1, ma), interior(p8, mb))
+
+
+def test_two_dimensional_run_matches_oracle():
+    """nz = 1: inactive third dimension (no ghosts, no sweep, CT only for the (x,y) pair)."""
+    n = 24
+    p = wl.default_params(nx=n, ny=n + 8, nz=1, ng=3, recon=wl.RECON_WENO5Z, riemann=wl.RIEMANN_HLL)
+    rng = np.random.default_rng(wl.SEED0 + 12)
+    q = np.zeros((8, 1, n + 8, n))
+    q[0] = 1.0 + 0.2 * rng.uniform(-1, 1, q[0].shape)
+    q[1:4] = 0.2 * rng.uniform(-1, 1, q[1:4].shape)
+    q[4] = 1.0 + 0.2 * rng.uniform(-1, 1, q[0].shape)
+    q[5:8] = 0.3 * rng.uniform(-1, 1, q[1:4].shape)
+    prim = wl.finish(p, q)
+    o, g = run_both(p, prim, nsteps=3)
+    compare(p, o, g, TOL_1STEP * 10)
+
+
+# ----------------------------------------------------------------------------- error behaviour of the C ABI
+def test_c_abi_rejects_bad_arguments():
+    torch, phx = _gpu()
+    p = wl.default_params(nx=16, ny=16, nz=16, ng=2, recon=wl.RECON_WENO5Z)
+    with pytest.raises(phx.PhxError) as e:
+        phx.init_mesh(p)                       # ng too small for WENO5-Z
+    assert e.value.code == phx.EINVAL
+    p = wl.default_params(nx=0, ny=16, nz=16)
+    with pytest.raises(phx.PhxError):
+        phx.init_mesh(p)
+    p = wl.default_params(nx=16, ny=16, nz=16, ng=2)
+    mesh = phx.init_mesh(p)
+    good = torch.zeros(mesh.field_elems, dtype=torch.float64, device="cuda")
+    with pytest.raises(phx.PhxError):
+        phx.prim_to_cons(mesh, good[:-8], good)            # wrong size (binding check)
+    rc = phx.lib().phx_prim_to_cons(mesh.handle, None, good.data_ptr(), None)
+    assert rc == phx.EINVAL and b"null" in phx.lib().phx_last_error()
+    rc = phx.lib().phx_prim_to_cons(mesh.handle, good.data_ptr() + 8, good.data_ptr(), None)
+    assert rc == phx.EINVAL                                  # misaligned
+    mesh.free()
+
+
+def test_evolve_host_matches_device_path():
+    torch, phx = _gpu()
+    w = WORKLOADS["cfg4_turb_24_weno"]
+    p = w["params"]
+    b = GpuRun(p, w["prim"])
+    t = 0.0
+    for _ in range(2):
+        b.phx.cfl_dt(b.mesh, b.prim, 0.4, b.d_dt)
+        t += float(b.d_dt.cpu())
+        b.phx.rk2_step(b.mesh, b.d_dt, b.cons0, b.cons, b.prim, b.mask)
+    cb, pb, _, mb = b.get()
+    mesh = phx.init_mesh(p)
+    hin = torch.from_numpy(w["prim"]).pin_memory()
+    hp = torch.empty_like(hin).pin_memory(); hc = torch.empty_like(hin).pin_memory()
+    hm = torch.empty(mb.shape, dtype=torch.uint8).pin_memory()
+    tt = phx.evolve_host(mesh, hin, 2, 0.4, hp, hc, hm)
+    assert tt == t
+    assert np.array_equal(hp.numpy(), pb) and np.array_equal(hc.numpy(), cb) and np.array_equal(hm.numpy(), mb)
