@@ -102,10 +102,10 @@ int phx_rk2_step(phx_mesh* mesh, const double* d_dt, double* d_cons0, double* d_
 int phx_evolve_host(phx_mesh* mesh, const double* h_prim_in, int nsteps, double cfl, double* h_prim_out,
                     double* h_cons_out, unsigned char* h_mask_out, double* h_t, void* stream);
 
-/* Face fluxes F~^d (after flux-CT is NOT applied; raw Riemann fluxes) of the last stage, for debugging and tests:
- * device pointer to the mesh-owned scratch of direction d (0,1,2), layout of one 8-variable field, the
- * face (i-1/2) stored at cell i. */
-const double* phx_debug_flux(const phx_mesh* mesh, int d);
+/* Raw Riemann face fluxes F~^d (before flux-CT) of the last stage, for debugging and tests: copies the mesh-owned
+ * scratch of direction d (0,1,2) into d_out (DEVICE, phx_field_elems doubles, layout of one 8-variable field,
+ * the face (i-1/2) stored at cell i), asynchronously on `stream`.  PHX_EINVAL for an inactive direction. */
+int phx_debug_flux(const phx_mesh* mesh, int d, double* d_out, void* stream);
 
 /* Count of this library's kernel launches since the mesh was created (for bench.py's gpu_launches). */
 unsigned long long phx_launch_count(const phx_mesh* mesh);

