@@ -1,0 +1,289 @@
+"""bench.py — GRMHD zone-cycles/s of the CUDA hot path on B200 (one JSON line on stdout).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 256]
+
+One "step" is one full RK2 cycle of the whole hot path over the whole mesh: phx_cfl_dt, then
+phx_rk2_step = U~0 copy + 2 x { x/y/z reconstruct+Riemann sweeps, flux-CT + divergence + sources + RK combine +
+con2prim + floors, ghost fill }.  Workload at N=1: BASELINE.json configs[3], the 256^3 periodic turbulence-like
+box (WENO5-Z, HLL, flux-CT, RK2, Minkowski, Gamma=5/3) that north_star's roofline target is quoted on; inputs are
+seeded synthetic fields from paper_2410_09146_b200/workloads.py (recipe in DESIGN.md section 4).
+
+value     : interior zones x K / device time (CUDA events, max over ranks), state resident in HBM.
+e2e       : same metric through phx_evolve_host (HOST buffers: H2D of the primitives and D2H of primitives,
+            conserved variables and mask inside the timed region, one call per step).
+roofline  : dominant kernel class, per-launch time from CUDA events recorded by the library on the launching
+            stream inside the timed region (phx_profile_*), algorithmic bytes / flops per zone from DESIGN.md 6.
+cpu_baseline : the oracle (oracle/, as it stands) on a bounded sample of the same workload on the host cores.
+N > 1     : the path does not shard in this build ("replicas only") - every rank runs an independent
+            replica of the same workload, no data-path collective; value = N x zones x K / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "grmhd_zone_cycles_per_sec"
+UNIT = "zone-cycles/s"
+
+# Algorithmic traffic and arithmetic per interior zone and launch (fp64 instruction counts from
+# the ncu capture profiles/r01_*.md, DFMA = 2 flop)
+ALGO_BYTES_PER_ZONE = {
+    "sweep_x": 128.0, "sweep_y": 128.0, "sweep_z": 128.0,       # read P (64 B), write F~ (64 B)
+    "update": 192.0 + 64.0 + 64.0 + 64.0 + 64.0 + 1.0,          # 3 fluxes, U~0, U~ in, U~ out, P out, mask
+    "fill_ghosts": 0.0, "cfl": 64.0, "prim_to_cons": 128.0, "c2p": 129.0, "copy": 128.0,
+}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n", type=int, default=256, help="zones per side of the config-4 box (256 = BASELINE.json)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                                       "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in self.f.read().splitlines():
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        self.f.close(); os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+# --------------------------------------------------------------------------------------------- the oracle, timed
+def oracle_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def time_oracle(n, steps):
+    """Zone-cycles/s of the CPU oracle (as it stands, OpenMP over its outer loops) on the config-4 recipe at n^3."""
+    from oracle import orc
+    from paper_2410_09146_b200 import workloads as wl
+    w = wl.turbulence_box(n)
+    o = orc.Run(w["params"], w["prim"])
+    per_step = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        dt = o.dt(w["cfl"])
+        o.step(dt)
+        per_step.append(time.perf_counter() - t0)
+    return wl.n_zones(w["params"]), per_step
+
+
+def run_reference(args):
+    """--impl reference: there is no reference code (PAPER.md only); the arm is the oracle on the host cores, each
+    step a bounded sample (a 64^3 box of the config-4 recipe) of the 256^3 workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = 64
+    zones, per_step = time_oracle(n, args.warmup + args.steps)
+    timed = per_step[args.warmup:]
+    total = sum(timed)
+    value = zones * len(timed) / total
+    cores = oracle_cores()
+    sample = f"config-4 recipe at {n}^3 (1/{(args.n // n) ** 3} of the {args.n}^3 workload), one RK2 step + CFL per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * total / len(timed), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"cfg4_turbulence_box_{args.n}^3_weno5z_hll_ct_rk2_minkowski", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------- the CUDA path
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2410_09146_b200 import phx, workloads as wl
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device - the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    phx.lib()   # fails loudly if libphx.so is missing
+
+    K, W = args.steps, max(args.warmup, 0)
+    w = wl.turbulence_box(args.n)
+    p = w["params"]
+    zones = wl.n_zones(p)
+    mesh = phx.init_mesh(p)
+    h_prim = torch.from_numpy(w["prim"])
+    prim = h_prim.cuda()
+    cons = torch.empty_like(prim); cons0 = torch.empty_like(prim)
+    mask = torch.zeros((prim.shape[0],) + tuple(prim.shape[2:]), dtype=torch.uint8, device="cuda")
+    d_dt = torch.zeros(1, dtype=torch.float64, device="cuda")
+    field_bytes = prim.numel() * 8
+    phx.prim_to_cons(mesh, prim, cons)
+
+    def step():
+        phx.cfl_dt(mesh, prim, w["cfl"], d_dt)
+        phx.rk2_step(mesh, d_dt, cons0, cons, prim, mask)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(W):
+        step()
+    barrier()
+    mesh.profile_enable(K * 12 + 8)
+    l0 = mesh.launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(K):
+        step()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    launches = mesh.launch_count() - l0
+    prof = mesh.profile_read()
+    mesh.profile_enable(0)
+    bad = int(mask.to(torch.int32).bitwise_and(16 | 32).count_nonzero().item())   # no-convergence / bad-input cells
+    finite = bool(torch.isfinite(cons).all().item())
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * zones * K / (ms * 1e-3)
+
+    # ---- end to end through the HOST-buffer C-ABI call (rank-local replica; max over ranks)
+    e2e = None
+    if not args.no_e2e:
+        del cons0
+        torch.cuda.empty_cache()
+        hin = h_prim.pin_memory()
+        hp = torch.empty_like(hin).pin_memory(); hc = torch.empty_like(hin).pin_memory()
+        hm = torch.empty(mask.shape, dtype=torch.uint8).pin_memory()
+        ke = max(1, min(K, 3))
+        phx.evolve_host(mesh, hin, 1, w["cfl"], hp, hc, hm)        # warm-up (allocates the workspace)
+        barrier()
+        e0.record()
+        for _ in range(ke):
+            phx.evolve_host(mesh, hin, 1, w["cfl"], hp, hc, hm)
+        e1.record()
+        barrier()
+        t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * zones * ke / (float(t.item()) * 1e-3), "unit": UNIT,
+               "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": 2 * field_bytes + hm.numel() + 16,
+               "steps": ke, "call": "phx_evolve_host(nsteps=1) per step, pinned host buffers"}
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel class
+    peaks, which = measured_peaks()
+    nall = int(np.prod(prim.shape)) // 8
+    per_launch_bytes = {k: v * zones for k, v in ALGO_BYTES_PER_ZONE.items()}
+    per_launch_bytes["fill_ghosts"] = (nall - zones) * 128.0
+    per_launch_bytes["update"] -= 32.0 * zones                       # stage 1 does not need a separate U~ (average of 2 stages)
+    kern = {k: {"ms_total": v[0], "launches": v[1], "ms_per_launch": v[0] / v[1], "share": v[0] / ms}
+            for k, v in prof.items() if v[1] > 0}
+    top = max(kern, key=lambda k: kern[k]["ms_total"])
+    dur = kern[top]["ms_per_launch"] * 1e-3
+    achieved = per_launch_bytes[top] / dur / 1e9
+    roofline = {"kernel": top, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": which,
+                "ms_per_launch": kern[top]["ms_per_launch"], "share_of_step": kern[top]["share"]}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"cfg4_turbulence_box_{args.n}^3_weno5z_hll_ct_rk2_minkowski", "zones": zones, "ng": p["ng"],
+                   "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no sharding)",
+                   "l2": f"inputs larger than L2 ({field_bytes / 1e6:.0f} MB per 8-variable field), no flush"},
+        "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "clocks": clocks,
+        "kernels": kern, "state_finite": finite, "c2p_failed_cells": bad,
+    }
+    if not args.no_cpu_baseline and world >= 1:
+        ns, steps = 96, 2
+        zs, per_step = time_oracle(ns, steps)
+        line["cpu_baseline"] = {"value": zs * steps / sum(per_step), "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
+                                "sample": f"config-4 recipe at {ns}^3, {steps} RK2 steps ({zs * steps} zone-cycles of the "
+                                          f"{zones * K} timed on the GPU)"}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -110,6 +110,16 @@ int phx_debug_flux(const phx_mesh* mesh, int d, double* d_out, void* stream);
 /* Count of this library's kernel launches since the mesh was created (for bench.py's gpu_launches). */
 unsigned long long phx_launch_count(const phx_mesh* mesh);
 
+/* Per-kernel-class timing with CUDA events recorded on the launching stream around every launch (bench.py's
+ * roofline figures).  phx_profile_enable(mesh, n) allocates n event pairs (n = 0 switches timing off); launches beyond
+ * n are not recorded.  phx_profile_read synchronises the recorded events, writes the summed milliseconds and the
+ * number of records per class into HOST arrays of PHX_K_COUNT entries, and resets the record list.
+ * PHX_K_CFL covers both reduction kernels of one phx_cfl_dt call; PHX_K_COPY is the U~0 <- U~ device copy of phx_rk2_step. */
+enum { PHX_K_SWEEP_X = 0, PHX_K_SWEEP_Y = 1, PHX_K_SWEEP_Z = 2, PHX_K_UPDATE = 3, PHX_K_FILL_GHOSTS = 4, PHX_K_CFL = 5,
+       PHX_K_PRIM_TO_CONS = 6, PHX_K_C2P = 7, PHX_K_COPY = 8, PHX_K_COUNT = 9 };
+int phx_profile_enable(phx_mesh* mesh, int max_records);
+int phx_profile_read(phx_mesh* mesh, double* h_ms, unsigned long long* h_count);
+
 const char* phx_last_error(void);
 
 #ifdef __cplusplus

@@ -427,6 +427,19 @@ struct phx_mesh {
   double* ws_field[3];
   unsigned char* ws_mask;
   double* ws_scal;   // [0] dt, [1] t
+  // per-kernel-class CUDA-event timing (phx_profile_enable / phx_profile_read)
+  cudaEvent_t* ev;   // 2 events per recorded launch
+  int* evcls;
+  int evcap, evn;
+};
+
+// RAII pair of events around one launch (or one group of launches) of class `cls`, recorded on the launching stream
+struct ProfScope {
+  phx_mesh* M; cudaStream_t st; int slot;
+  ProfScope(phx_mesh* M_, int cls, cudaStream_t st_) : M(M_), st(st_), slot(-1) {
+    if (M->ev && M->evn < M->evcap) { slot = M->evn++; M->evcls[slot] = cls; cudaEventRecord(M->ev[2 * slot], st); }
+  }
+  ~ProfScope() { if (slot >= 0) cudaEventRecord(M->ev[2 * slot + 1], st); }
 };
 
 static thread_local char g_err[512] = "";
@@ -522,6 +535,7 @@ extern "C" int phx_free_mesh(phx_mesh* M) {
   for (int d = 0; d < 3; ++d) if (M->ws_field[d]) cudaFree(M->ws_field[d]);
   if (M->ws_mask) cudaFree(M->ws_mask);
   if (M->ws_scal) cudaFree(M->ws_scal);
+  if (M->ev) { for (int i = 0; i < 2 * M->evcap; ++i) cudaEventDestroy(M->ev[i]); delete[] M->ev; delete[] M->evcls; }
   delete M;
   return PHX_OK;
 }
@@ -546,9 +560,12 @@ extern "C" int phx_prim_to_cons(const phx_mesh* Mc, const double* d_prim, double
   if (!M || !aligned16(d_prim) || !aligned16(d_cons)) return fail(PHX_EINVAL, "phx_prim_to_cons: null or misaligned argument");
   cudaStream_t st = (cudaStream_t)stream;
   const unsigned nb = (unsigned)((M->nall + 255) / 256);
+  {
+  ProfScope ps(M, PHX_K_PRIM_TO_CONS, st);
 #define CALL(MET) k_prim_to_cons<MET><<<nb, 256, 0, st>>>(M->m, d_prim, d_cons, M->nall)
   DISPATCH_METRIC(M, CALL);
 #undef CALL
+  }
   LAUNCH_CHECK(M, "k_prim_to_cons");
   return PHX_OK;
 }
@@ -557,7 +574,8 @@ extern "C" int phx_fill_ghosts(const phx_mesh* Mc, double* d_prim, void* stream)
   phx_mesh* M = const_cast<phx_mesh*>(Mc);
   if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
   if (M->nall == M->ninterior) return PHX_OK;
-  k_fill_ghosts<<<(unsigned)((M->nall + 255) / 256), 256, 0, (cudaStream_t)stream>>>(M->m, d_prim, M->nall);
+  { ProfScope ps(M, PHX_K_FILL_GHOSTS, (cudaStream_t)stream);
+    k_fill_ghosts<<<(unsigned)((M->nall + 255) / 256), 256, 0, (cudaStream_t)stream>>>(M->m, d_prim, M->nall); }
   LAUNCH_CHECK(M, "k_fill_ghosts");
   return PHX_OK;
 }
@@ -567,11 +585,14 @@ extern "C" int phx_cons_to_prim(const phx_mesh* Mc, double* d_cons, double* d_pr
   if (!M || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask) return fail(PHX_EINVAL, "phx_cons_to_prim: null or misaligned argument");
   cudaStream_t st = (cudaStream_t)stream;
   const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
+  {
+  ProfScope ps(M, PHX_K_C2P, st);
 #define CALL(MET)                                                                                         \
   if (M->m.excise) k_c2p<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior); \
   else k_c2p<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior)
   DISPATCH_METRIC(M, CALL);
 #undef CALL
+  }
   LAUNCH_CHECK(M, "k_c2p");
   return phx_fill_ghosts(M, d_prim, stream);
 }
@@ -589,6 +610,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int rowlen = m.n[0] + 2;
     const long long npos = (long long)m.nblk * cnt[2] * cnt[1] * rowlen;
     const unsigned nb = (unsigned)((npos + (XS_BLOCK - 2)) / (XS_BLOCK - 1));
+    ProfScope ps(M, PHX_K_SWEEP_X, st);
     k_sweep_x<METRIC, RECON><<<nb, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], npos, rowlen, cnt[1], cnt[2], lo[1], lo[2]);
     M->launches++;
   }
@@ -599,6 +621,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int L = (nfaces + nseg - 1) / nseg;
     const int ntr = cnt[0] * cnt[2];
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, m.nblk * nseg);
+    ProfScope ps(M, PHX_K_SWEEP_Y, st);
     k_sweep_march<METRIC, RECON, 1><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], nseg, L);
     M->launches++;
   }
@@ -608,6 +631,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int L = (nfaces + nseg - 1) / nseg;
     const int ntr = cnt[0] * cnt[1];
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, m.nblk * nseg);
+    ProfScope ps(M, PHX_K_SWEEP_Z, st);
     k_sweep_march<METRIC, RECON, 2><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], nseg, L);
     M->launches++;
   }
@@ -634,11 +658,14 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
   FluxPtrs fl;
   for (int d = 0; d < 3; ++d) fl.f[d] = M->flux[d];
   const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
+  {
+  ProfScope ps(M, PHX_K_UPDATE, st);
 #define CALL(MET)                                                                                                                   \
   if (M->m.excise) k_update<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons, d_prim, d_mask, M->ninterior); \
   else k_update<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons, d_prim, d_mask, M->ninterior)
   DISPATCH_METRIC(M, CALL);
 #undef CALL
+  }
   LAUNCH_CHECK(M, "k_update");
   return phx_fill_ghosts(M, d_prim, st);
 }
@@ -656,7 +683,8 @@ extern "C" int phx_rk2_step(phx_mesh* M, const double* d_dt, double* d_cons0, do
     return fail(PHX_EINVAL, "phx_rk2_step: null, misaligned or aliased argument");
   cudaStream_t st = (cudaStream_t)stream;
   // U~0 <- U~, then both stages in place on d_cons
-  CUDA_TRY(cudaMemcpyAsync(d_cons0, d_cons, (size_t)M->nall * NV * sizeof(double), cudaMemcpyDeviceToDevice, st), "cudaMemcpyAsync");
+  { ProfScope ps(M, PHX_K_COPY, st);
+    CUDA_TRY(cudaMemcpyAsync(d_cons0, d_cons, (size_t)M->nall * NV * sizeof(double), cudaMemcpyDeviceToDevice, st), "cudaMemcpyAsync"); }
   int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons0, d_cons, d_prim, d_mask, st);
   if (rc != PHX_OK) return rc;
   return stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons0, d_cons, d_prim, d_mask, st);
@@ -668,6 +696,8 @@ extern "C" int phx_cfl_dt(const phx_mesh* Mc, const double* d_prim, double cfl, 
   cudaStream_t st = (cudaStream_t)stream;
   long long want = (M->ninterior + 255) / 256;
   const int nb = (int)(want < M->npartial ? want : M->npartial);
+  {
+  ProfScope ps(M, PHX_K_CFL, st);
 #define CALL(MET)                                                                                          \
   if (M->m.excise) k_cfl_partial<MET, true><<<nb, 256, 0, st>>>(M->m, M->xfl, d_prim, M->partial, M->ninterior); \
   else k_cfl_partial<MET, false><<<nb, 256, 0, st>>>(M->m, M->xfl, d_prim, M->partial, M->ninterior)
@@ -676,10 +706,39 @@ extern "C" int phx_cfl_dt(const phx_mesh* Mc, const double* d_prim, double cfl, 
   LAUNCH_CHECK(M, "k_cfl_partial");
   k_cfl_final<<<1, 256, 0, st>>>(M->partial, nb, cfl, d_dt);
   LAUNCH_CHECK(M, "k_cfl_final");
+  }
   if (h_dt) {
     CUDA_TRY(cudaMemcpyAsync(h_dt, d_dt, sizeof(double), cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
     CUDA_TRY(cudaStreamSynchronize(st), "cudaStreamSynchronize");
   }
+  return PHX_OK;
+}
+
+// ---- per-kernel-class event timing ------------------------------------------------------------------------------
+extern "C" int phx_profile_enable(phx_mesh* M, int max_records) {
+  if (!M || max_records < 0) return fail(PHX_EINVAL, "phx_profile_enable: null mesh or negative capacity");
+  if (M->ev) { for (int i = 0; i < 2 * M->evcap; ++i) cudaEventDestroy(M->ev[i]); delete[] M->ev; delete[] M->evcls; M->ev = nullptr; M->evcls = nullptr; }
+  M->evcap = M->evn = 0;
+  if (max_records == 0) return PHX_OK;
+  M->ev = new (std::nothrow) cudaEvent_t[2 * (size_t)max_records];
+  M->evcls = new (std::nothrow) int[max_records];
+  if (!M->ev || !M->evcls) { delete[] M->ev; delete[] M->evcls; M->ev = nullptr; M->evcls = nullptr; return fail(PHX_ENOMEM, "phx_profile_enable: host allocation failed"); }
+  for (int i = 0; i < 2 * max_records; ++i) CUDA_TRY(cudaEventCreate(&M->ev[i]), "cudaEventCreate");
+  M->evcap = max_records;
+  return PHX_OK;
+}
+
+extern "C" int phx_profile_read(phx_mesh* M, double* h_ms, unsigned long long* h_count) {
+  if (!M || !h_ms || !h_count) return fail(PHX_EINVAL, "phx_profile_read: null argument");
+  for (int c = 0; c < PHX_K_COUNT; ++c) { h_ms[c] = 0.0; h_count[c] = 0; }
+  for (int i = 0; i < M->evn; ++i) {
+    CUDA_TRY(cudaEventSynchronize(M->ev[2 * i + 1]), "cudaEventSynchronize");
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, M->ev[2 * i], M->ev[2 * i + 1]), "cudaEventElapsedTime");
+    h_ms[M->evcls[i]] += ms;
+    h_count[M->evcls[i]]++;
+  }
+  M->evn = 0;
   return PHX_OK;
 }
 

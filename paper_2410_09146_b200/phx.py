@@ -18,10 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libphx.so")
 OK, EINVAL, ECUDA, ENOMEM, EUNSUPPORTED = 0, 1, 2, 3, 4
 M_RHO_FLOOR, M_EPS_FLOOR, M_EPS_CLIPPED, M_W_CEIL, M_NOCONV, M_BAD_INPUT, M_EXCISED = 1, 2, 4, 8, 16, 32, 64
 
+KERNEL_CLASSES = ("sweep_x", "sweep_y", "sweep_z", "update", "fill_ghosts", "cfl", "prim_to_cons", "c2p", "copy")
+
 EXPORTS = (
     "phx_init_mesh", "phx_free_mesh", "phx_field_elems", "phx_mask_elems", "phx_prim_to_cons",
     "phx_cons_to_prim", "phx_fill_ghosts", "phx_rk_stage", "phx_cfl_dt", "phx_rk2_step",
     "phx_evolve_host", "phx_debug_flux", "phx_launch_count", "phx_last_error",
+    "phx_profile_enable", "phx_profile_read",
 )
 
 
@@ -84,6 +87,8 @@ def lib():
         L.phx_evolve_host.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp, vp, C.POINTER(C.c_double), vp]
         L.phx_debug_flux.argtypes = [vp, C.c_int, dp, vp]
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
+        L.phx_profile_enable.argtypes = [vp, C.c_int]
+        L.phx_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
         L.phx_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -130,6 +135,15 @@ class Mesh:
         out = torch.empty(shape, dtype=torch.float64, device="cuda")
         _check(lib().phx_debug_flux(self.handle, int(d), _dev(out, torch.float64, self.field_elems, "out"), _stream(stream)))
         return out
+
+    def profile_enable(self, max_records):
+        _check(lib().phx_profile_enable(self.handle, int(max_records)))
+
+    def profile_read(self):
+        """{kernel class: (summed ms, records)} of the launches recorded since the last read."""
+        ms = (C.c_double * len(KERNEL_CLASSES))(); n = (C.c_ulonglong * len(KERNEL_CLASSES))()
+        _check(lib().phx_profile_read(self.handle, ms, n))
+        return {k: (ms[i], int(n[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
     def free(self):
         if self._h:
