@@ -41,6 +41,15 @@ ALGO_BYTES_PER_ZONE = {
     "update": 192.0 + 64.0 + 64.0 + 64.0 + 64.0 + 1.0,          # 3 fluxes, U~0, U~ in, U~ out, P out, mask
     "fill_ghosts": 0.0, "cfl": 64.0, "prim_to_cons": 128.0, "c2p": 129.0, "copy": 128.0,
 }
+# fp64 flop per interior zone and launch for the WENO5-Z + HLL Minkowski path: dadd + dmul + 2*dfma thread-instructions of
+# the round-1 implementation counted by ncu (profiles/r01_ncu_summary.md), frozen as the algorithmic figure
+ALGO_FLOP_PER_ZONE = {"sweep_x": 1400.0, "sweep_y": 1419.0, "sweep_z": 1419.0, "update": 1758.0, "cfl": 173.0}
+# fp64 peak from unit counts and clocks: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz; a DFMA loop measured
+# 33.9 TFLOP/s on this pool's B200 (16.94 T DFMA/s)
+FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+FP64_MEASURED_DFMA_TFLOPS = 33.9
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (bytes)
+NCU_TRAFFIC = {256: {"update": 7.286e9, "sweep_x": 2.206e9, "sweep_y": 2.381e9, "sweep_z": 2.379e9}}
 
 
 def parse_args():
@@ -256,10 +265,22 @@ def run_ours(args):
             for k, v in prof.items() if v[1] > 0}
     top = max(kern, key=lambda k: kern[k]["ms_total"])
     dur = kern[top]["ms_per_launch"] * 1e-3
-    achieved = per_launch_bytes[top] / dur / 1e9
-    roofline = {"kernel": top, "bound": "hbm", "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": which,
-                "ms_per_launch": kern[top]["ms_per_launch"], "share_of_step": kern[top]["share"]}
+    hbm = per_launch_bytes[top] / dur / 1e9
+    flops = ALGO_FLOP_PER_ZONE.get(top, 0.0) * zones / dur / 1e12
+    traffic = NCU_TRAFFIC.get(args.n, {}).get(top)
+    if flops / FP64_PEAK_TFLOPS >= hbm / peaks["hbm_gbs"]:
+        roofline = {"kernel": top, "bound": "alu", "achieved": flops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": flops / FP64_PEAK_TFLOPS, "traffic": traffic,
+                    "peak_source": "derived: 148 SM x 64 fp64 lanes x 2 x 1.965 GHz (DFMA loop measured %.1f)" % FP64_MEASURED_DFMA_TFLOPS,
+                    "hbm_gbs_achieved": hbm, "hbm_frac": hbm / peaks["hbm_gbs"]}
+    else:
+        roofline = {"kernel": top, "bound": "hbm", "achieved": hbm, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                    "frac": hbm / peaks["hbm_gbs"], "traffic": traffic, "peak_source": which,
+                    "fp64_tflops_achieved": flops, "fp64_frac": flops / FP64_PEAK_TFLOPS}
+    roofline.update(ms_per_launch=kern[top]["ms_per_launch"], share_of_step=kern[top]["share"])
+    # whole-step fp64 fraction: algorithmic flop of all launches of one step / step time
+    step_flop = 2.0 * sum(ALGO_FLOP_PER_ZONE[k] for k in ("sweep_x", "sweep_y", "sweep_z", "update")) + ALGO_FLOP_PER_ZONE["cfl"]
+    roofline["step_fp64_frac"] = step_flop * zones / (ms / K * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
