@@ -1,0 +1,156 @@
+"""Full-size GPU parity: BASELINE.json's configs at their full sizes, in the launch configuration bench.py times
+(phx_cfl_dt with the time step kept on the device + phx_rk2_step), checked
+
+  (i)  on sampled outputs the oracle can compute one by one: the update of a cell depends on the primitives within
+       HALO = 8 cells (two stages x (3 cells of WENO5 stencil to a face + 1 transverse cell of flux-CT)), so the oracle
+       run on a (16+2*HALO)^3 sub-box cut around a sample point reproduces the central 16^3 cells of the full run
+       exactly (sub-box faces that coincide with an outflow domain face carry the true boundary condition and are
+       valid up to the face); and
+  (ii) via properties that hold at any size: corner-centred div(sqrt(gamma) B) unchanged, totals conserved on the
+       periodic box, state finite, no con2prim failure bits.
+
+Tolerance: BASELINE.json's 1e-11 relative per conserved variable after one RK2 step, scale = max |U~_v| over the whole
+mesh (SURVEY.md 8c error metric), identical masks on the sampled cells.
+"""
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2410_09146_b200 import workloads as wl
+
+from harness import GpuRun, TOL_1STEP
+
+pytestmark = pytest.mark.gpu
+
+HALO = 8
+CORE = 16
+
+
+def sub_box(p, q_glob, origin):
+    """Cut a (CORE+2*HALO)^3 box with lower corner `origin` (global interior indices, x y z) out of the global interior
+    array q_glob [8, Nz, Ny, Nx]; periodic axes wrap, outflow axes must stay inside the domain.  Returns (p_sub, prim)."""
+    s = CORE + 2 * HALO
+    N = (q_glob.shape[3], q_glob.shape[2], q_glob.shape[1])
+    idx = []
+    for d in range(3):
+        i = np.arange(origin[d], origin[d] + s)
+        if p["bc"][d][0] == wl.BC_PERIODIC:
+            i = i % N[d]
+        assert i.min() >= 0 and i.max() < N[d]
+        idx.append(i)
+    q = q_glob[:, idx[2]][:, :, idx[1]][:, :, :, idx[0]]
+    ps = dict(p)
+    dx = [(p["xmax"][d] - p["xmin"][d]) / N[d] for d in range(3)]
+    ps.update(nbx=1, nby=1, nbz=1, nx=s, ny=s, nz=s,
+              xmin=tuple(p["xmin"][d] + origin[d] * dx[d] for d in range(3)),
+              xmax=tuple(p["xmin"][d] + (origin[d] + s) * dx[d] for d in range(3)))
+    return ps, wl.finish(ps, np.ascontiguousarray(q))
+
+
+def valid_range(p, origin, N):
+    """Per axis: slice of sub-box interior cells whose full-mesh update the sub-box reproduces."""
+    s = CORE + 2 * HALO
+    out = []
+    for d in range(3):
+        lo, hi = HALO, s - HALO
+        if p["bc"][d][0] == wl.BC_OUTFLOW:
+            if origin[d] == 0:
+                lo = 0
+            if origin[d] + s == N[d]:
+                hi = s
+        out.append(slice(lo, hi))
+    return out
+
+
+def corner_div(Bt, rdx):
+    """Corner-centred divergence of a densitised field, numpy [3, Nz, Ny, Nx] -> [Nz-1, Ny-1, Nx-1]."""
+    def mu(a, ax):
+        n = a.shape[ax]
+        return 0.5 * (np.take(a, range(0, n - 1), axis=ax) + np.take(a, range(1, n), axis=ax))
+
+    def de(a, ax):
+        n = a.shape[ax]
+        return np.take(a, range(1, n), axis=ax) - np.take(a, range(0, n - 1), axis=ax)
+    X, Y, Z = 2, 1, 0
+    return (de(mu(mu(Bt[0], Y), Z), X) * rdx[0] + de(mu(mu(Bt[1], X), Z), Y) * rdx[1] + de(mu(mu(Bt[2], X), Y), Z) * rdx[2])
+
+
+def run_full(w, origins, check_conservation):
+    import torch
+    p = w["params"]
+    q_glob = wl.from_blocks(p, w["prim"])
+    N = (q_glob.shape[3], q_glob.shape[2], q_glob.shape[1])
+    g = GpuRun(p, w["prim"])
+    gx, gy, gz = wl.ghosts(p)
+    rdx = [N[d] / (p["xmax"][d] - p["xmin"][d]) for d in range(3)]
+    c0 = wl.from_blocks(p, g.cons.cpu().numpy())
+    div0 = corner_div(c0[5:8], rdx)
+    dt_ref = orc.cfl_dt(p, w["prim"], w["cfl"])
+    g.step_device_dt(w["cfl"])                       # phx_cfl_dt (device dt) + phx_rk2_step: what bench.py times
+    dt_gpu = float(g.d_dt.cpu())
+    assert abs(dt_gpu - dt_ref) <= 1e-13 * dt_ref
+    cons, prim, _, mask = g.get()
+    assert np.isfinite(cons[:, :, gz:gz + p["nz"], gy:gy + p["ny"], gx:gx + p["nx"]]).all()
+    assert not (mask & (16 | 32)).any(), "con2prim failure bits at full size"
+    cg = wl.from_blocks(p, cons)
+    mg = wl.from_blocks(p, mask[:, None])[0]
+    scale = np.abs(cg).reshape(8, -1).max(axis=1)
+    ddiv = np.abs(corner_div(cg[5:8], rdx) - div0).max()
+    bscale = np.abs(c0[5:8]).max() * max(rdx)
+    assert ddiv <= 1e-13 * bscale, f"corner div B changed by {ddiv} (scale {bscale})"
+    if check_conservation:
+        rel = np.abs(np.sum(cg - c0, axis=(1, 2, 3), dtype=np.longdouble)) / np.sum(np.abs(c0), axis=(1, 2, 3))
+        assert rel.max() <= 1e-13, f"totals drifted by {rel}"
+    del c0, div0
+    worst = np.zeros(8)
+    for origin in origins:
+        ps, sprim = sub_box(p, q_glob, origin)
+        orc.reset_c2p_margin()
+        o = orc.Run(ps, sprim)
+        o.step(dt_ref)
+        assert orc.last_c2p_margin() > 1e-9
+        oc = wl.from_blocks(ps, o.cons); om = wl.from_blocks(ps, o.mask[:, None])[0]
+        vr = valid_range(p, origin, N)
+        sl_sub = (slice(None), vr[2], vr[1], vr[0])
+        gi = [np.arange(origin[d] + vr[d].start, origin[d] + vr[d].stop) % N[d] for d in range(3)]
+        got = cg[:, gi[2]][:, :, gi[1]][:, :, :, gi[0]]
+        gm = mg[gi[2]][:, gi[1]][:, :, gi[0]]
+        err = np.abs(got - oc[sl_sub]).reshape(8, -1).max(axis=1) / scale
+        worst = np.maximum(worst, err)
+        assert err.max() <= TOL_1STEP, f"sub-box at {origin}: errors {err}"
+        assert np.array_equal(gm, om[sl_sub[1:]]), f"sub-box at {origin}: masks differ"
+    print(w["name"], "full size, worst sampled error per variable", worst)
+    g.mesh.free()
+    del g
+    torch.cuda.empty_cache()
+
+
+def test_cfg4_turbulence_256_sampled():
+    """BASELINE.json configs[3], the bench workload: 256^3 periodic, WENO5-Z + HLL + flux-CT."""
+    w = wl.turbulence_box(256)
+    n, s = 256, CORE + 2 * HALO
+    origins = [(0, 0, 0), (n - HALO - 3, 100, n - 20), (117, n - s // 2, 5), (64, 200, 131), (201, 37, 88)]
+    run_full(w, origins, check_conservation=True)
+
+
+def test_cfg2_periodic_box_64_sampled():
+    """BASELINE.json configs[1]: 64^3 periodic, PLM-MC + LLF + flux-CT."""
+    w = wl.periodic_box(64)
+    run_full(w, [(0, 0, 0), (50, 20, 40), (30, 60, 7)], check_conservation=True)
+
+
+def test_cfg3_kerr_schild_128_sampled():
+    """BASELINE.json configs[2]: 128^3 Kerr-Schild torus with excision (sub-boxes: a domain corner with its outflow
+    faces, the excised region at the centre, the torus body)."""
+    w = wl.kerr_schild_torus(128)
+    n, s = 128, CORE + 2 * HALO
+    run_full(w, [(0, 0, 0), (n - s, n - s, n - s), (48, 48, 48), (80, 50, 52), (20, 60, 56)], check_conservation=False)
+
+
+def test_cfg5_packed_blocks_512x32_sampled():
+    """BASELINE.json configs[4]: 512 blocks of 32^3 in one batched launch per kernel; sub-boxes straddle block faces,
+    edges and corners (the oracle runs them as one block: block invariance is pin P11)."""
+    w = wl.packed_blocks((8, 8, 8), 32)
+    n, s = 256, CORE + 2 * HALO
+    run_full(w, [(0, 0, 0), (n - s, n - s, n - s), (112, 112, 112), (16, 48, 80), (150, 100, 120), (176, 16, 208)],
+             check_conservation=False)
