@@ -221,14 +221,17 @@ __global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, con
   int cb[3];
   block_coords(m, b, cb);
   const double x = xcen(m, 0, cb[0], i), y = xcen(m, 1, cb[1], j), z = xcen(m, 2, cb[2], k);
+  double U[NV], q[NV];
+  // stage-input primitives of this cell: sources, and the initial guess of the con2prim root
+  q[RHO] = prim[vb + RHO * m.ncell + c];
+  q[UX] = prim[vb + UX * m.ncell + c]; q[UY] = prim[vb + UY * m.ncell + c]; q[UZ] = prim[vb + UZ * m.ncell + c];
+  q[UU] = prim[vb + UU * m.ncell + c];
   if constexpr (METRIC == 1) {
-    double q[NV], S[4];
-#pragma unroll
-    for (int v = 0; v < NV; ++v) q[v] = prim[vb + v * m.ncell + c];
+    double S[4];
+    q[BX] = prim[vb + BX * m.ncell + c]; q[BY] = prim[vb + BY * m.ncell + c]; q[BZ] = prim[vb + BZ * m.ncell + c];
     ks_sources(m, x, y, z, q, S);
     R[CS1] += S[0]; R[CS2] += S[1]; R[CS3] += S[2]; R[CTAU] += S[3];
   }
-  double U[NV], q[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     const long long id = vb + v * m.ncell + c;
@@ -236,7 +239,8 @@ __global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, con
   }
   Geo<METRIC> G;
   G.at(m, x, y, z);
-  const unsigned char mk = c2p_cell<METRIC>(m, G, U, q);
+  const double mu_guess = c2p_guess<METRIC>(G, q, m.gam);
+  const unsigned char mk = c2p_cell<METRIC>(m, G, U, q, mu_guess);
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     const long long id = vb + v * m.ncell + c;
