@@ -46,22 +46,21 @@ __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G
 // position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
 template <int METRIC, int RECON>
 __global__ void __launch_bounds__(XS_BLOCK) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
-                                                      long long npos, int rowlen, int nrj, int nrk, int j0, int k0) {
+                                                      int nplane, int rowlen, int j0, int k0) {
+  // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii)
   constexpr int HW = ReconTraits<RECON>::HW;
   __shared__ double sh[NV][XS_BLOCK];
   const int t = threadIdx.x;
-  const long long p = (long long)blockIdx.x * (XS_BLOCK - 1) + t;
-  const bool valid = p < npos;
+  const int p = blockIdx.x * (XS_BLOCK - 1) + t;
+  const bool valid = p < nplane;
   double qm[NV], qp[NV];
   long long base = 0;
-  int ii = 0, i = 0, j = 0, k = 0, b = 0;
+  int ii = 0, i = 0, j = 0, k = 0;
+  const int b = blockIdx.z;
   if (valid) {
-    const long long row = p / rowlen;
-    ii = (int)(p - row * rowlen);
-    const int jj = (int)(row % nrj);
-    const long long r2 = row / nrj;
-    const int kk = (int)(r2 % nrk);
-    b = (int)(r2 / nrk);
+    const int kk = blockIdx.y;
+    const int jj = p / rowlen;
+    ii = p - jj * rowlen;
     i = m.g[0] - 1 + ii; j = j0 + jj; k = k0 + kk;
     base = (long long)b * NV * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
     double centre[NV];
@@ -178,13 +177,13 @@ __global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, con
                                                      double bdt_host, const double* __restrict__ d_dt, double beta,
                                                      const double* cons0, double* cons,
                                                      double* __restrict__ prim, unsigned char* __restrict__ mask, long long ninterior) {
-  const long long p = (long long)blockIdx.x * UP_BLOCK + threadIdx.x;
-  if (p >= ninterior) return;
-  const int ii = (int)(p % m.n[0]);
-  long long r = p / m.n[0];
-  const int jj = (int)(r % m.n[1]); r /= m.n[1];
-  const int kk = (int)(r % m.n[2]);
-  const int b = (int)(r / m.n[2]);
+  // blockIdx.z = block, blockIdx.y = kk selects one interior k-plane; the plane is tiled flat over (jj, ii)
+  const int p = blockIdx.x * UP_BLOCK + threadIdx.x;
+  if (p >= m.n[0] * m.n[1]) return;
+  const int jj = p / m.n[0];
+  const int ii = p - jj * m.n[0];
+  const int b = blockIdx.z;
+  const int kk = blockIdx.y;
   const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
   const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
   const long long vb = (long long)b * NV * m.ncell;     // block offset in an 8-variable field
@@ -509,6 +508,11 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   M->nall = (long long)m.nblk * m.ncell;
   M->ninterior = (long long)m.nblk * m.n[0] * m.n[1] * m.n[2];
   if (M->nall * NV >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
+  // launch geometry: blocks ride on gridDim.z, k-planes or sweep segments on gridDim.y (both limited to 65535)
+  if (m.nblk > 65535 || m.na[2] > 65535 || (long long)m.nblk * ((m.n[1] > m.n[2] ? m.n[1] : m.n[2]) / 33 + 2) > 65535 ||
+      (long long)m.na[0] * m.na[1] >= (1LL << 31)) {
+    delete M; return fail(PHX_EUNSUPPORTED, "phx_init_mesh: more than 65535 blocks or k-planes, or a k-plane of 2^31 cells");
+  }
   const size_t fbytes = (size_t)M->nall * NV * sizeof(double);
   cudaStream_t st = (cudaStream_t)stream;
   for (int d = 0; d < 3; ++d) {
@@ -612,10 +616,10 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
   }
   if (m.act[0]) {
     const int rowlen = m.n[0] + 2;
-    const long long npos = (long long)m.nblk * cnt[2] * cnt[1] * rowlen;
-    const unsigned nb = (unsigned)((npos + (XS_BLOCK - 2)) / (XS_BLOCK - 1));
+    const int nplane = cnt[1] * rowlen;
+    dim3 grid((nplane + (XS_BLOCK - 2)) / (XS_BLOCK - 1), cnt[2], m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_X, st);
-    k_sweep_x<METRIC, RECON><<<nb, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], npos, rowlen, cnt[1], cnt[2], lo[1], lo[2]);
+    k_sweep_x<METRIC, RECON><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], nplane, rowlen, lo[1], lo[2]);
     M->launches++;
   }
   const int Lmax = 33;
@@ -661,7 +665,7 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
   { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
   FluxPtrs fl;
   for (int d = 0; d < 3; ++d) fl.f[d] = M->flux[d];
-  const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
+  const dim3 nb((M->m.n[0] * M->m.n[1] + UP_BLOCK - 1) / UP_BLOCK, M->m.n[2], M->m.nblk);
   {
   ProfScope ps(M, PHX_K_UPDATE, st);
 #define CALL(MET)                                                                                                                   \
