@@ -88,8 +88,9 @@ int phx_rk_stage(phx_mesh* mesh, double g0, double g1, double beta_dt, const dou
  * and the stream is synchronised. */
 int phx_cfl_dt(const phx_mesh* mesh, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream);
 
-/* One full RK2 step with the time step read from the device scalar d_dt (no host round trip):
- * copies U~ to d_cons0, runs both stages; equivalent to two phx_rk_stage calls. */
+/* One full RK2 step with the time step read from the device scalar d_dt (no host round trip); the result equals two
+ * phx_rk_stage calls bit for bit.  d_cons0 is scratch (same size as d_cons, must not alias it): stage 1 writes its
+ * state U~1 there, stage 2 combines U~0 = d_cons and U~1 into d_cons; on return d_cons0 holds U~1. */
 int phx_rk2_step(phx_mesh* mesh, const double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
                  unsigned char* d_mask, void* stream);
 
@@ -114,7 +115,7 @@ unsigned long long phx_launch_count(const phx_mesh* mesh);
  * roofline figures).  phx_profile_enable(mesh, n) allocates n event pairs (n = 0 switches timing off); launches beyond
  * n are not recorded.  phx_profile_read synchronises the recorded events, writes the summed milliseconds and the
  * number of records per class into HOST arrays of PHX_K_COUNT entries, and resets the record list.
- * PHX_K_CFL covers both reduction kernels of one phx_cfl_dt call; PHX_K_COPY is the U~0 <- U~ device copy of phx_rk2_step. */
+ * PHX_K_CFL covers both reduction kernels of one phx_cfl_dt call; PHX_K_COPY is unused (phx_rk2_step makes no copy). */
 enum { PHX_K_SWEEP_X = 0, PHX_K_SWEEP_Y = 1, PHX_K_SWEEP_Z = 2, PHX_K_UPDATE = 3, PHX_K_FILL_GHOSTS = 4, PHX_K_CFL = 5,
        PHX_K_PRIM_TO_CONS = 6, PHX_K_C2P = 7, PHX_K_COPY = 8, PHX_K_COUNT = 9 };
 int phx_profile_enable(phx_mesh* mesh, int max_records);

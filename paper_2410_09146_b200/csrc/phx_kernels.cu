@@ -18,9 +18,28 @@
 using namespace phx;
 
 // ================================================================================================ kernels
-constexpr int XS_BLOCK = 128;   // threads per block of the x sweep (XS_BLOCK-1 faces per block)
-constexpr int MS_BLOCK = 128;   // threads per block of the marching sweeps
-constexpr int UP_BLOCK = 128;
+// launch shapes (tuned on B200 with ncu, profiles/): threads per block and minimum resident blocks per SM
+#ifndef PHX_XS_BLOCK
+#define PHX_XS_BLOCK 128
+#endif
+#ifndef PHX_XS_MINB
+#define PHX_XS_MINB 1
+#endif
+#ifndef PHX_MS_BLOCK
+#define PHX_MS_BLOCK 128
+#endif
+#ifndef PHX_MS_MINB
+#define PHX_MS_MINB 2
+#endif
+#ifndef PHX_UP_BLOCK
+#define PHX_UP_BLOCK 128
+#endif
+#ifndef PHX_UP_MINB
+#define PHX_UP_MINB 6      // Minkowski update: HBM-bound, wants resident warps (80 registers); Kerr-Schild keeps its registers
+#endif
+constexpr int XS_BLOCK = PHX_XS_BLOCK;   // threads per block of the x sweep (XS_BLOCK-1 faces per block)
+constexpr int MS_BLOCK = PHX_MS_BLOCK;   // threads per block of the marching sweeps
+constexpr int UP_BLOCK = PHX_UP_BLOCK;
 
 template <int RECON>
 __device__ __forceinline__ void positivity_fallback(const MeshDev& m, const double* centre, double* qm, double* qp) {
@@ -45,7 +64,7 @@ __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G
 // ---- x sweep ------------------------------------------------------------------------------------
 // position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
 template <int METRIC, int RECON>
-__global__ void __launch_bounds__(XS_BLOCK) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+__global__ void __launch_bounds__(XS_BLOCK, PHX_XS_MINB) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
                                                       int nplane, int rowlen, int j0, int k0) {
   // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii)
   constexpr int HW = ReconTraits<RECON>::HW;
@@ -94,7 +113,7 @@ __global__ void __launch_bounds__(XS_BLOCK) k_sweep_x(MeshDev m, const double* _
 // ---- y / z sweep ---------------------------------------------------------------------------------
 // transverse position p -> (t1, t0) with t0 along x (fastest); blockIdx.y = b*nseg + segment.
 template <int METRIC, int RECON, int D>
-__global__ void __launch_bounds__(MS_BLOCK) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+__global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
                                                           int ntr, int n0, int lo0, int lo1, int nseg, int L) {
   constexpr int HW = ReconTraits<RECON>::HW;
   const int p = blockIdx.x * MS_BLOCK + threadIdx.x;
@@ -173,10 +192,12 @@ __device__ __forceinline__ void ct_pair(const MeshDev& m, const FluxPtrs& fl, co
 }
 
 template <int METRIC, bool EXC>
-__global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
+__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : 1)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                                      double bdt_host, const double* __restrict__ d_dt, double beta,
-                                                     const double* cons0, double* cons,
-                                                     double* __restrict__ prim, unsigned char* __restrict__ mask, long long ninterior) {
+                                                     const double* cons0, const double* cons_in, double* cons_out,
+                                                     double* __restrict__ prim, unsigned char* __restrict__ mask) {
+  // U~_out = g0 U~0 + g1 U~_in + bdt R.  cons_out may alias cons_in or cons0 (every thread touches only its own cell of
+  // the conserved fields); cons_in is not read when g1 == 0 (first stage).
   // blockIdx.z = block, blockIdx.y = kk selects one interior k-plane; the plane is tiled flat over (jj, ii)
   const int p = blockIdx.x * UP_BLOCK + threadIdx.x;
   if (p >= m.n[0] * m.n[1]) return;
@@ -189,7 +210,15 @@ __global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, con
   const long long vb = (long long)b * NV * m.ncell;     // block offset in an 8-variable field
   const long long fb = (long long)b * m.ncell;          // block offset in a one-variable field
   if (EXC) {
-    if (xfl[fb + c] & XF_CELL) { mask[fb + c] = M_EXCISED; return; }
+    if (xfl[fb + c] & XF_CELL) {   // frozen cell: the RK combination of two equal states is exact
+#pragma unroll
+      for (int v = 0; v < NV; ++v) {
+        const long long id = vb + v * m.ncell + c;
+        cons_out[id] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] : cons0[id];
+      }
+      mask[fb + c] = M_EXCISED;
+      return;
+    }
   }
   const double bdt = d_dt ? beta * (*d_dt) : bdt_host;
   const long long str[3] = {1, m.sj, m.sk};
@@ -234,7 +263,7 @@ __global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, con
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     const long long id = vb + v * m.ncell + c;
-    U[v] = g0 * cons0[id] + g1 * cons[id] + bdt * R[v];
+    U[v] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] + bdt * R[v] : g0 * cons0[id] + bdt * R[v];
   }
   Geo<METRIC> G;
   G.at(m, x, y, z);
@@ -243,7 +272,7 @@ __global__ void __launch_bounds__(UP_BLOCK) k_update(MeshDev m, FluxPtrs fl, con
 #pragma unroll
   for (int v = 0; v < NV; ++v) {
     const long long id = vb + v * m.ncell + c;
-    cons[id] = U[v];
+    cons_out[id] = U[v];
     prim[id] = q[v];
   }
   mask[fb + c] = mk;
@@ -660,7 +689,7 @@ static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
 }
 
 static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
-                      double* d_cons, double* d_prim, unsigned char* d_mask, cudaStream_t st) {
+                      const double* d_cons_in, double* d_cons_out, double* d_prim, unsigned char* d_mask, cudaStream_t st) {
   launch_sweeps(M, d_prim, st);
   { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
   FluxPtrs fl;
@@ -669,8 +698,8 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
   {
   ProfScope ps(M, PHX_K_UPDATE, st);
 #define CALL(MET)                                                                                                                   \
-  if (M->m.excise) k_update<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons, d_prim, d_mask, M->ninterior); \
-  else k_update<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons, d_prim, d_mask, M->ninterior)
+  if (M->m.excise) k_update<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask); \
+  else k_update<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask)
   DISPATCH_METRIC(M, CALL);
 #undef CALL
   }
@@ -682,7 +711,7 @@ extern "C" int phx_rk_stage(phx_mesh* M, double g0, double g1, double beta_dt, c
                             unsigned char* d_mask, void* stream) {
   if (!M || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask)
     return fail(PHX_EINVAL, "phx_rk_stage: null or misaligned argument");
-  return stage_impl(M, g0, g1, beta_dt, nullptr, 0.0, d_cons0, d_cons, d_prim, d_mask, (cudaStream_t)stream);
+  return stage_impl(M, g0, g1, beta_dt, nullptr, 0.0, d_cons0, d_cons, d_cons, d_prim, d_mask, (cudaStream_t)stream);
 }
 
 extern "C" int phx_rk2_step(phx_mesh* M, const double* d_dt, double* d_cons0, double* d_cons, double* d_prim, unsigned char* d_mask,
@@ -690,12 +719,10 @@ extern "C" int phx_rk2_step(phx_mesh* M, const double* d_dt, double* d_cons0, do
   if (!M || !d_dt || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask || d_cons0 == d_cons)
     return fail(PHX_EINVAL, "phx_rk2_step: null, misaligned or aliased argument");
   cudaStream_t st = (cudaStream_t)stream;
-  // U~0 <- U~, then both stages in place on d_cons
-  { ProfScope ps(M, PHX_K_COPY, st);
-    CUDA_TRY(cudaMemcpyAsync(d_cons0, d_cons, (size_t)M->nall * NV * sizeof(double), cudaMemcpyDeviceToDevice, st), "cudaMemcpyAsync"); }
-  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons0, d_cons, d_prim, d_mask, st);
+  // no copy of U~0: stage 1 reads U~0 = d_cons and writes U~1 into the scratch field; stage 2 combines both into d_cons
+  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st);
   if (rc != PHX_OK) return rc;
-  return stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons0, d_cons, d_prim, d_mask, st);
+  return stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons, d_cons0, d_cons, d_prim, d_mask, st);
 }
 
 extern "C" int phx_cfl_dt(const phx_mesh* Mc, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream) {
