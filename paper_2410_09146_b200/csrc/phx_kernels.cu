@@ -26,10 +26,10 @@ using namespace phx;
 #define PHX_XS_MINB 1
 #endif
 #ifndef PHX_MS_BLOCK
-#define PHX_MS_BLOCK 128
+#define PHX_MS_BLOCK 64
 #endif
 #ifndef PHX_MS_MINB
-#define PHX_MS_MINB 2
+#define PHX_MS_MINB 6
 #endif
 #ifndef PHX_UP_BLOCK
 #define PHX_UP_BLOCK 128
@@ -111,16 +111,32 @@ __global__ void __launch_bounds__(XS_BLOCK, PHX_XS_MINB) k_sweep_x(MeshDev m, co
 }
 
 // ---- y / z sweep ---------------------------------------------------------------------------------
-// transverse position p -> (t1, t0) with t0 along x (fastest); blockIdx.y = b*nseg + segment.
+// Lanes along x (coalesced); every thread marches along the sweep direction over one segment of faces.  The (2*HW+1)-row
+// stencil window of its column lives in shared memory as a ring of rows that cp.async fills one row ahead of the
+// arithmetic (each primitive is read from HBM once per segment, no register window, no long-scoreboard stall); a thread
+// reads only its own column of the ring, so no block barrier is needed, only cp.async.wait_group.
+// transverse position p -> (t1, t0) with t0 along x (fastest); blockIdx.y = segment, blockIdx.z = block.
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 template <int METRIC, int RECON, int D>
 __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
-                                                          int ntr, int n0, int lo0, int lo1, int nseg, int L) {
+                                                                       int ntr, int n0, int lo0, int lo1, int L) {
   constexpr int HW = ReconTraits<RECON>::HW;
-  const int p = blockIdx.x * MS_BLOCK + threadIdx.x;
+  constexpr int NW = 2 * HW + 1;   // stencil rows
+  constexpr int NR = NW + 1;       // ring: the stencil plus one row in flight
+  __shared__ double win[NR][NV][MS_BLOCK];
+  const int tid = threadIdx.x;
+  const int p = blockIdx.x * MS_BLOCK + tid;
   if (p >= ntr) return;
-  const int b = blockIdx.y / nseg;
-  const int seg = blockIdx.y - b * nseg;
-  const int t0 = p % n0, t1 = p / n0;
+  const int b = blockIdx.z;
+  const int seg = blockIdx.y;
+  const int t1 = p / n0, t0 = p - t1 * n0;
   const int i = lo0 + t0;             // x index
   const int o = lo1 + t1;             // the other transverse index (k for D=1, j for D=2)
   const long long sd = (D == 1) ? m.sj : m.sk;
@@ -134,26 +150,46 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
   const double xx = xcen(m, 0, cb[0], i);
   const double xo = (D == 1) ? xcen(m, 2, cb[2], o) : xcen(m, 1, cb[1], o);
 
-  double w[2 * HW + 1][NV];
+  const int rlast = f1 + HW;                      // last row any cell of this segment needs
+  const double* src = prim + col + (long long)(f0 - 1 - HW) * sd;   // row f0-1-HW of this column
+  // prologue: rows of the first cell's stencil, one commit group per row
 #pragma unroll
-  for (int r = 0; r < 2 * HW; ++r)
+  for (int r = 0; r < NW; ++r) {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) w[r][v] = prim[col + v * m.ncell + (long long)(f0 - 1 - HW + r) * sd];
+    for (int v = 0; v < NV; ++v) cp_async8(&win[r][v][tid], src + v * m.ncell);
+    cp_async_commit();
+    src += sd;
+  }
+  int s0 = 0;                                     // ring slot of row c-HW
+  int snew = NW;                                  // ring slot the next prefetched row goes to
   double qpPrev[NV];
 #pragma unroll
   for (int v = 0; v < NV; ++v) qpPrev[v] = 0.0;
   for (int c = f0 - 1; c <= f1; ++c) {
+    if (c + HW + 1 <= rlast) {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) w[2 * HW][v] = prim[col + v * m.ncell + (long long)(c + HW) * sd];
-    double qm[NV], qp[NV];
+      for (int v = 0; v < NV; ++v) cp_async8(&win[snew][v][tid], src + v * m.ncell);
+      src += sd;
+    }
+    cp_async_commit();
+    cp_async_wait<1>();                           // everything but the row just issued has landed
+    const double* wrow[NW];
+#pragma unroll
+    for (int r = 0; r < NW; ++r) {
+      int sl = s0 + r;
+      sl = (sl >= NR) ? sl - NR : sl;
+      wrow[r] = &win[sl][0][tid];
+    }
+    double qm[NV], qp[NV], centre[NV];
 #pragma unroll
     for (int v = 0; v < NV; ++v) {
-      double f[2 * HW + 1];
+      double f[NW];
 #pragma unroll
-      for (int s = 0; s <= 2 * HW; ++s) f[s] = w[s][v];
+      for (int r = 0; r < NW; ++r) f[r] = wrow[r][v * MS_BLOCK];
+      centre[v] = f[HW];
       recon1<RECON>(f, qm[v], qp[v]);
     }
-    positivity_fallback<RECON>(m, w[HW], qm, qp);
+    positivity_fallback<RECON>(m, centre, qm, qp);
     if (c >= f0) {
       Geo<METRIC> G;
       const double xf = xface(m, D, cb[D], c);
@@ -165,11 +201,10 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
     }
 #pragma unroll
     for (int v = 0; v < NV; ++v) qpPrev[v] = qp[v];
-#pragma unroll
-    for (int r = 0; r < 2 * HW; ++r)
-#pragma unroll
-      for (int v = 0; v < NV; ++v) w[r][v] = w[r + 1][v];
+    s0 = (s0 + 1 == NR) ? 0 : s0 + 1;
+    snew = (snew + 1 == NR) ? 0 : snew + 1;
   }
+  cp_async_wait<0>();
 }
 
 // ---- update: flux-CT + divergence + sources + RK combine + con2prim + floors ----------------------
@@ -538,7 +573,7 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   M->ninterior = (long long)m.nblk * m.n[0] * m.n[1] * m.n[2];
   if (M->nall * NV >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
   // launch geometry: blocks ride on gridDim.z, k-planes or sweep segments on gridDim.y (both limited to 65535)
-  if (m.nblk > 65535 || m.na[2] > 65535 || (long long)m.nblk * ((m.n[1] > m.n[2] ? m.n[1] : m.n[2]) / 33 + 2) > 65535 ||
+  if (m.nblk > 65535 || m.na[2] > 65535 ||
       (long long)m.na[0] * m.na[1] >= (1LL << 31)) {
     delete M; return fail(PHX_EUNSUPPORTED, "phx_init_mesh: more than 65535 blocks or k-planes, or a k-plane of 2^31 cells");
   }
@@ -657,9 +692,9 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int nseg = (nfaces + Lmax - 1) / Lmax;
     const int L = (nfaces + nseg - 1) / nseg;
     const int ntr = cnt[0] * cnt[2];
-    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, m.nblk * nseg);
+    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Y, st);
-    k_sweep_march<METRIC, RECON, 1><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], nseg, L);
+    k_sweep_march<METRIC, RECON, 1><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], L);
     M->launches++;
   }
   if (m.act[2]) {
@@ -667,9 +702,9 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int nseg = (nfaces + Lmax - 1) / Lmax;
     const int L = (nfaces + nseg - 1) / nseg;
     const int ntr = cnt[0] * cnt[1];
-    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, m.nblk * nseg);
+    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Z, st);
-    k_sweep_march<METRIC, RECON, 2><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], nseg, L);
+    k_sweep_march<METRIC, RECON, 2><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], L);
     M->launches++;
   }
 }
