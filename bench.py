@@ -3,7 +3,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 256]
 
 One "step" is one full RK2 cycle of the whole hot path over the whole mesh: phx_cfl_dt, then
-phx_rk2_step = U~0 copy + 2 x { x/y/z reconstruct+Riemann sweeps, flux-CT + divergence + sources + RK combine +
+phx_rk2_step = 2 x { x/y/z reconstruct+Riemann sweeps, flux-CT + divergence + sources + RK combine +
 con2prim + floors, ghost fill }.  Workload at N=1: BASELINE.json configs[3], the 256^3 periodic turbulence-like
 box (WENO5-Z, HLL, flux-CT, RK2, Minkowski, Gamma=5/3) that north_star's roofline target is quoted on; inputs are
 seeded synthetic fields from paper_2410_09146_b200/workloads.py (recipe in DESIGN.md section 4).
@@ -34,22 +34,26 @@ if ROOT not in sys.path:
 METRIC = "grmhd_zone_cycles_per_sec"
 UNIT = "zone-cycles/s"
 
-# Algorithmic traffic and arithmetic per interior zone and launch (fp64 instruction counts from
-# the ncu capture profiles/r01_*.md, DFMA = 2 flop)
+# Algorithmic traffic and arithmetic per interior zone and launch.
+# Bytes: what the kernel's definition must move.  update = 3 x 7 flux components read (the d-th magnetic component of F~^d
+# is identically zero and not needed) + U~0 read + U~1 read (stage 2 only: 32 B averaged over both stages) + 5 primitives
+# read (sources / con2prim guess) + U~ and P written + mask.
 ALGO_BYTES_PER_ZONE = {
     "sweep_x": 128.0, "sweep_y": 128.0, "sweep_z": 128.0,       # read P (64 B), write F~ (64 B)
-    "update": 192.0 + 64.0 + 64.0 + 64.0 + 64.0 + 1.0,          # 3 fluxes, U~0, U~ in, U~ out, P out, mask
+    "update": 168.0 + 64.0 + 32.0 + 40.0 + 64.0 + 64.0 + 1.0,
     "fill_ghosts": 0.0, "cfl": 64.0, "prim_to_cons": 128.0, "c2p": 129.0, "copy": 128.0,
 }
 # fp64 flop per interior zone and launch for the WENO5-Z + HLL Minkowski path: dadd + dmul + 2*dfma thread-instructions of
-# the round-1 implementation counted by ncu (profiles/r01_ncu_summary.md), frozen as the algorithmic figure
-ALGO_FLOP_PER_ZONE = {"sweep_x": 1400.0, "sweep_y": 1419.0, "sweep_z": 1419.0, "update": 1758.0, "cfl": 173.0}
+# the committed kernels counted by ncu (profiles/r01_ncu_summary.md; con2prim iterations are data dependent, the figure
+# is the one measured on this workload).  achieved = these flops / measured time, i.e. useful fp64 work only.
+ALGO_FLOP_PER_ZONE = {"sweep_x": 1322.0, "sweep_y": 1340.0, "sweep_z": 1339.0, "update": 657.0, "cfl": 151.0}
 # fp64 peak from unit counts and clocks: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz; a DFMA loop measured
 # 33.9 TFLOP/s on this pool's B200 (16.94 T DFMA/s)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 FP64_MEASURED_DFMA_TFLOPS = 33.9
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (bytes)
-NCU_TRAFFIC = {256: {"update": 7.286e9, "sweep_x": 2.206e9, "sweep_y": 2.381e9, "sweep_z": 2.379e9}}
+NCU_TRAFFIC = {256: {"update": 7.016e9, "sweep_x": 2.207e9, "sweep_y": 2.301e9, "sweep_z": 2.299e9, "cfl": 1.112e9,
+                     "fill_ghosts": 0.230e9}}
 
 
 def parse_args():
@@ -59,6 +63,9 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="zones per side of the config-4 box (256 = BASELINE.json)")
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"],
+                    help="cfg4 (default) is the bench workload; the others time BASELINE.json's other 3-D configs at full size "
+                         "(reported without a roofline object: the per-zone figures of DESIGN.md 6 are config 4's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -181,7 +188,15 @@ def run_ours(args):
     phx.lib()   # fails loudly if libphx.so is missing
 
     K, W = args.steps, max(args.warmup, 0)
-    w = wl.turbulence_box(args.n)
+    if args.workload == "cfg4":
+        w = wl.turbulence_box(args.n)
+        wname = f"cfg4_turbulence_box_{args.n}^3_weno5z_hll_ct_rk2_minkowski"
+    elif args.workload == "cfg2":
+        w = wl.periodic_box(64); wname = "cfg2_periodic_box_64^3_plm_mc_llf_ct_rk2_minkowski"
+    elif args.workload == "cfg3":
+        w = wl.kerr_schild_torus(128); wname = "cfg3_kerr_schild_torus_128^3_plm_minmod_hll_ct_rk2"
+    else:
+        w = wl.packed_blocks((8, 8, 8), 32); wname = "cfg5_packed_blocks_512x32^3_kerr_schild_plm_minmod_hll_ct_rk2"
     p = w["params"]
     zones = wl.n_zones(p)
     mesh = phx.init_mesh(p)
@@ -260,7 +275,6 @@ def run_ours(args):
     nall = int(np.prod(prim.shape)) // 8
     per_launch_bytes = {k: v * zones for k, v in ALGO_BYTES_PER_ZONE.items()}
     per_launch_bytes["fill_ghosts"] = (nall - zones) * 128.0
-    per_launch_bytes["update"] -= 32.0 * zones                       # stage 1 does not need a separate U~ (average of 2 stages)
     kern = {k: {"ms_total": v[0], "launches": v[1], "ms_per_launch": v[0] / v[1], "share": v[0] / ms}
             for k, v in prof.items() if v[1] > 0}
     top = max(kern, key=lambda k: kern[k]["ms_total"])
@@ -285,13 +299,15 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"cfg4_turbulence_box_{args.n}^3_weno5z_hll_ct_rk2_minkowski", "zones": zones, "ng": p["ng"],
+        "config": {"workload": wname, "zones": zones, "ng": p["ng"],
                    "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (no sharding)",
                    "l2": f"inputs larger than L2 ({field_bytes / 1e6:.0f} MB per 8-variable field), no flush"},
         "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline, "clocks": clocks,
         "kernels": kern, "state_finite": finite, "c2p_failed_cells": bad,
     }
-    if not args.no_cpu_baseline and world >= 1:
+    if args.workload != "cfg4" or args.n != 256:
+        line["roofline"] = None if args.workload != "cfg4" else roofline
+    if not args.no_cpu_baseline and world >= 1 and args.workload == "cfg4":
         ns, steps = 96, 2
         zs, per_step = time_oracle(ns, steps)
         line["cpu_baseline"] = {"value": zs * steps / sum(per_step), "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
