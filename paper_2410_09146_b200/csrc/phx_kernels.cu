@@ -37,6 +37,9 @@ using namespace phx;
 #ifndef PHX_UP_MINB
 #define PHX_UP_MINB 6      // Minkowski update: HBM-bound, wants resident warps (80 registers); Kerr-Schild keeps its registers
 #endif
+#ifndef PHX_UP_MINB_KS
+#define PHX_UP_MINB_KS 4
+#endif
 constexpr int XS_BLOCK = PHX_XS_BLOCK;   // threads per block of the x sweep (XS_BLOCK-1 faces per block)
 constexpr int MS_BLOCK = PHX_MS_BLOCK;   // threads per block of the marching sweeps
 constexpr int UP_BLOCK = PHX_UP_BLOCK;
@@ -227,7 +230,7 @@ __device__ __forceinline__ void ct_pair(const MeshDev& m, const FluxPtrs& fl, co
 }
 
 template <int METRIC, bool EXC>
-__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : 1)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
+__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : PHX_UP_MINB_KS)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                                      double bdt_host, const double* __restrict__ d_dt, double beta,
                                                      const double* cons0, const double* cons_in, double* cons_out,
                                                      double* __restrict__ prim, unsigned char* __restrict__ mask) {
@@ -369,15 +372,15 @@ __global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* _
 }
 
 // ---- ghost fill: one gather pass -------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, long long nall) {
-  const long long p = (long long)blockIdx.x * 256 + threadIdx.x;
-  if (p >= nall) return;
+// blockIdx.z = block, blockIdx.y = allocated k-plane, the plane is tiled flat over (j, i); interior cells leave at once.
+__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim) {
+  const int p = blockIdx.x * 256 + threadIdx.x;
+  if (p >= m.na[0] * m.na[1]) return;
   int l[3];
-  l[0] = (int)(p % m.na[0]);
-  long long r = p / m.na[0];
-  l[1] = (int)(r % m.na[1]); r /= m.na[1];
-  l[2] = (int)(r % m.na[2]);
-  const int b = (int)(r / m.na[2]);
+  l[1] = p / m.na[0];
+  l[0] = p - l[1] * m.na[0];
+  l[2] = blockIdx.y;
+  const int b = blockIdx.z;
   bool interior = true;
 #pragma unroll
   for (int d = 0; d < 3; ++d) interior = interior && (l[d] >= m.g[d]) && (l[d] < m.g[d] + m.n[d]);
@@ -386,17 +389,29 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restri
   block_coords(m, b, cb);
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    int gi = cb[d] * m.n[d] + (l[d] - m.g[d]);
-    if (gi < 0) gi = (m.bc[d][0] == 0) ? gi + m.N[d] : 0;
-    else if (gi >= m.N[d]) gi = (m.bc[d][1] == 0) ? gi - m.N[d] : m.N[d] - 1;
-    sb[d] = gi / m.n[d];
-    sl[d] = gi - sb[d] * m.n[d] + m.g[d];
+    // source cell in block-local terms: inside this block, in the neighbour block, wrapped or clamped at a domain face
+    int li = l[d] - m.g[d];            // -g .. n+g-1
+    int nbk = cb[d];
+    if (li < 0) {
+      if (nbk > 0) { nbk -= 1; li += m.n[d]; }
+      else if (m.bc[d][0] == 0) { nbk = m.nb[d] - 1; li += m.n[d]; }
+      else li = 0;
+    } else if (li >= m.n[d]) {
+      if (nbk < m.nb[d] - 1) { nbk += 1; li -= m.n[d]; }
+      else if (m.bc[d][1] == 0) { nbk = 0; li -= m.n[d]; }
+      else li = m.n[d] - 1;
+    }
+    sb[d] = nbk;
+    sl[d] = li + m.g[d];
   }
   const int bs = (sb[2] * m.nb[1] + sb[1]) * m.nb[0] + sb[0];
   const long long src = (long long)bs * NV * m.ncell + (long long)sl[2] * m.sk + (long long)sl[1] * m.sj + sl[0];
   const long long dst = (long long)b * NV * m.ncell + (long long)l[2] * m.sk + (long long)l[1] * m.sj + l[0];
+  double v[NV];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) prim[dst + v * m.ncell] = prim[src + v * m.ncell];
+  for (int q = 0; q < NV; ++q) v[q] = prim[src + q * m.ncell];
+#pragma unroll
+  for (int q = 0; q < NV; ++q) prim[dst + q * m.ncell] = v[q];
 }
 
 // ---- CFL: warp-shuffle min reduction ------------------------------------------------------------------
@@ -647,7 +662,8 @@ extern "C" int phx_fill_ghosts(const phx_mesh* Mc, double* d_prim, void* stream)
   if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
   if (M->nall == M->ninterior) return PHX_OK;
   { ProfScope ps(M, PHX_K_FILL_GHOSTS, (cudaStream_t)stream);
-    k_fill_ghosts<<<(unsigned)((M->nall + 255) / 256), 256, 0, (cudaStream_t)stream>>>(M->m, d_prim, M->nall); }
+    const dim3 grid((M->m.na[0] * M->m.na[1] + 255) / 256, M->m.na[2], M->m.nblk);
+    k_fill_ghosts<<<grid, 256, 0, (cudaStream_t)stream>>>(M->m, d_prim); }
   LAUNCH_CHECK(M, "k_fill_ghosts");
   return PHX_OK;
 }
