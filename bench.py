@@ -2,9 +2,9 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--n 256]
 
-One "step" is one full RK2 cycle of the whole hot path over the whole mesh: phx_cfl_dt, then
-phx_rk2_step = 2 x { x/y/z reconstruct+Riemann sweeps, flux-CT + divergence + sources + RK combine +
-con2prim + floors, ghost fill }.  Workload at N=1: BASELINE.json configs[3], the 256^3 periodic turbulence-like
+One "step" is one full RK2 cycle of the whole hot path over the whole mesh: phx_rk2_step_cfl =
+2 x { x/y/z reconstruct+Riemann sweeps, flux-CT + divergence + sources + RK combine + con2prim + floors, ghost fill }
+with the CFL reduction of the next time step fused into the second stage's update kernel (a8/a7 of SURVEY.md 8a).  Workload at N=1: BASELINE.json configs[3], the 256^3 periodic turbulence-like
 box (WENO5-Z, HLL, flux-CT, RK2, Minkowski, Gamma=5/3) that north_star's roofline target is quoted on; inputs are
 seeded synthetic fields from paper_2410_09146_b200/workloads.py (recipe in DESIGN.md section 4).
 
@@ -208,9 +208,10 @@ def run_ours(args):
     field_bytes = prim.numel() * 8
     phx.prim_to_cons(mesh, prim, cons)
 
+    phx.cfl_dt(mesh, prim, w["cfl"], d_dt)      # dt of the first step; every later dt comes out of the step itself
+
     def step():
-        phx.cfl_dt(mesh, prim, w["cfl"], d_dt)
-        phx.rk2_step(mesh, d_dt, cons0, cons, prim, mask)
+        phx.rk2_step_cfl(mesh, w["cfl"], d_dt, cons0, cons, prim, mask)
 
     def barrier():
         if world > 1:

@@ -94,8 +94,14 @@ int phx_cfl_dt(const phx_mesh* mesh, const double* d_prim, double cfl, double* d
 int phx_rk2_step(phx_mesh* mesh, const double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
                  unsigned char* d_mask, void* stream);
 
+/* phx_rk2_step followed by phx_cfl_dt on the new primitives, with the reduction fused into the second stage's update
+ * kernel: on entry *d_dt (device) is the time step of this step, on return it is cfl * min 1/sum_d max|lambda^d|/dx_d of the
+ * state the step produced -- the same bits phx_cfl_dt would write.  Start a run with one phx_cfl_dt call. */
+int phx_rk2_step_cfl(phx_mesh* mesh, double cfl, double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
+                     unsigned char* d_mask, void* stream);
+
 /* HOST-buffer path (the end-to-end call): copies h_prim_in (HOST, phx_field_elems doubles, ghosts filled) to
- * mesh-owned device fields, computes U~ (phx_prim_to_cons), then runs `nsteps` times { phx_cfl_dt ; phx_rk2_step }
+ * mesh-owned device fields, computes U~ (phx_prim_to_cons), then runs phx_cfl_dt once and `nsteps` times phx_rk2_step_cfl
  * with the time step kept on the device, and copies the primitives (required), the conserved variables and the
  * last stage's mask (both nullable) back to HOST buffers.  *h_t (nullable) receives the elapsed coordinate time.
  * Synchronises `stream` before returning.  The device workspace (3 fields + mask) is allocated on first use and

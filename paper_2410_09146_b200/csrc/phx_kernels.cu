@@ -229,16 +229,18 @@ __device__ __forceinline__ void ct_pair(const MeshDev& m, const FluxPtrs& fl, co
   dB[A] -= (-0.5 * (e01 + e11) + 0.5 * (e00 + e10)) * m.rdx[C];
 }
 
-template <int METRIC, bool EXC>
-__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : PHX_UP_MINB_KS)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
-                                                     double bdt_host, const double* __restrict__ d_dt, double beta,
-                                                     const double* cons0, const double* cons_in, double* cons_out,
-                                                     double* __restrict__ prim, unsigned char* __restrict__ mask) {
+// One cell of the update.  Returns sum_d max|lambda^d|/dx_d of the new primitives when CFL is set (0 for a thread without
+// a cell or with an excised one), so that the kernel can reduce the next time step on the fly.
+template <int METRIC, bool EXC, bool CFL>
+__device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& fl, const unsigned char* __restrict__ xfl, double g0, double g1,
+                                              double bdt_host, const double* __restrict__ d_dt, double beta,
+                                              const double* cons0, const double* cons_in, double* cons_out,
+                                              double* __restrict__ prim, unsigned char* __restrict__ mask) {
   // U~_out = g0 U~0 + g1 U~_in + bdt R.  cons_out may alias cons_in or cons0 (every thread touches only its own cell of
   // the conserved fields); cons_in is not read when g1 == 0 (first stage).
   // blockIdx.z = block, blockIdx.y = kk selects one interior k-plane; the plane is tiled flat over (jj, ii)
   const int p = blockIdx.x * UP_BLOCK + threadIdx.x;
-  if (p >= m.n[0] * m.n[1]) return;
+  if (p >= m.n[0] * m.n[1]) return 0.0;
   const int jj = p / m.n[0];
   const int ii = p - jj * m.n[0];
   const int b = blockIdx.z;
@@ -255,7 +257,7 @@ __global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : PHX_UP_
         cons_out[id] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] : cons0[id];
       }
       mask[fb + c] = M_EXCISED;
-      return;
+      return 0.0;
     }
   }
   const double bdt = d_dt ? beta * (*d_dt) : bdt_host;
@@ -314,6 +316,58 @@ __global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : PHX_UP_
     prim[id] = q[v];
   }
   mask[fb + c] = mk;
+  if constexpr (CFL) {
+    double lam[3];
+    max_speeds<METRIC>(q, G, m.gam, lam);
+    double sum = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) if (m.act[d]) sum += lam[d] * m.rdx[d];
+    return sum;
+  }
+  return 0.0;
+}
+
+// smax: PHX_NSLOT accumulators of the largest sum_d max|lambda^d|/dx_d seen (bit pattern of a non-negative double, which
+// orders like the unsigned integer), one atomicMax per thread block; k_cfl_final_slots turns them into the time step.
+constexpr int PHX_NSLOT = 1024;
+template <int METRIC, bool EXC, bool CFL>
+__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : PHX_UP_MINB_KS)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
+                                                     double bdt_host, const double* __restrict__ d_dt, double beta,
+                                                     const double* cons0, const double* cons_in, double* cons_out,
+                                                     double* __restrict__ prim, unsigned char* __restrict__ mask,
+                                                     unsigned long long* __restrict__ smax) {
+  double sum = update_cell<METRIC, EXC, CFL>(m, fl, xfl, g0, g1, bdt_host, d_dt, beta, cons0, cons_in, cons_out, prim, mask);
+  if constexpr (CFL) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sum = fmax(sum, __shfl_xor_sync(0xffffffffu, sum, o));
+    __shared__ double sh[UP_BLOCK / 32];
+    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = sum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double v = sh[0];
+#pragma unroll
+      for (int w = 1; w < UP_BLOCK / 32; ++w) v = fmax(v, sh[w]);
+      const unsigned slot = (blockIdx.x + blockIdx.y * gridDim.x + blockIdx.z * gridDim.x * gridDim.y) % PHX_NSLOT;
+      atomicMax(&smax[slot], (unsigned long long)__double_as_longlong(v));
+    }
+  }
+}
+
+// dt = cfl / max over the slots; the slots are reset for the next accumulation
+__global__ void __launch_bounds__(256) k_cfl_final_slots(unsigned long long* __restrict__ smax, double cfl, double* __restrict__ dt) {
+  double best = 0.0;
+  for (int p = threadIdx.x; p < PHX_NSLOT; p += 256) { best = fmax(best, __longlong_as_double((long long)smax[p])); smax[p] = 0ull; }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
+  __shared__ double sh[8];
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double v = sh[0];
+#pragma unroll
+    for (int w = 1; w < 8; ++w) v = fmax(v, sh[w]);
+    *dt = cfl * (1.0 / v);
+  }
 }
 
 // ---- stand-alone con2prim, prim->cons ---------------------------------------------------------------
@@ -418,7 +472,9 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restri
 template <int METRIC, bool EXC>
 __global__ void __launch_bounds__(256) k_cfl_partial(MeshDev m, const unsigned char* __restrict__ xfl, const double* __restrict__ prim,
                                                      double* __restrict__ partial, long long ninterior) {
-  double best = INFINITY;
+  // max of sum_d max|lambda^d|/dx_d; the final kernel takes cfl * (1/max), which equals cfl * min(1/sum) bit for bit
+  // because IEEE division is monotone
+  double best = 0.0;
   for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < ninterior; p += (long long)gridDim.x * 256) {
     const int ii = (int)(p % m.n[0]);
     long long r = p / m.n[0];
@@ -439,34 +495,34 @@ __global__ void __launch_bounds__(256) k_cfl_partial(MeshDev m, const unsigned c
     double s = 0.0;
 #pragma unroll
     for (int d = 0; d < 3; ++d) if (m.act[d]) s += lam[d] * m.rdx[d];
-    best = fmin(best, 1.0 / s);
+    best = fmax(best, s);
   }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
   __shared__ double sh[8];
   if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
   __syncthreads();
   if (threadIdx.x < 32) {
-    double v = (threadIdx.x < 8) ? sh[threadIdx.x] : INFINITY;
+    double v = (threadIdx.x < 8) ? sh[threadIdx.x] : 0.0;
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    for (int o = 4; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     if (threadIdx.x == 0) partial[blockIdx.x] = v;
   }
 }
 
 __global__ void __launch_bounds__(256) k_cfl_final(const double* __restrict__ partial, int n, double cfl, double* __restrict__ dt) {
-  double best = INFINITY;
-  for (int p = threadIdx.x; p < n; p += 256) best = fmin(best, partial[p]);
+  double best = 0.0;
+  for (int p = threadIdx.x; p < n; p += 256) best = fmax(best, partial[p]);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) best = fmin(best, __shfl_xor_sync(0xffffffffu, best, o));
+  for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
   __shared__ double sh[8];
   if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = best;
   __syncthreads();
   if (threadIdx.x < 32) {
-    double v = (threadIdx.x < 8) ? sh[threadIdx.x] : INFINITY;
+    double v = (threadIdx.x < 8) ? sh[threadIdx.x] : 0.0;
 #pragma unroll
-    for (int o = 4; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
-    if (threadIdx.x == 0) *dt = cfl * v;
+    for (int o = 4; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if (threadIdx.x == 0) *dt = cfl * (1.0 / v);
   }
 }
 
@@ -503,6 +559,7 @@ struct phx_mesh {
   unsigned char* xfl;
   double* partial;
   int npartial;
+  unsigned long long* smax;   // PHX_NSLOT accumulators of the fused CFL reduction (zero between steps)
   unsigned long long launches;
   long long nall, ninterior;
   // workspace of the host-buffer path (phx_evolve_host), allocated on first use
@@ -603,6 +660,8 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   }
   M->npartial = 148 * 8;
   if (cudaMalloc((void**)&M->partial, sizeof(double) * M->npartial) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
+  if (cudaMalloc((void**)&M->smax, sizeof(unsigned long long) * PHX_NSLOT) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
+  if (cudaMemsetAsync(M->smax, 0, sizeof(unsigned long long) * PHX_NSLOT, st) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ECUDA, "phx_init_mesh: cudaMemsetAsync failed"); }
   if (m.excise) {
     if (cudaMalloc((void**)&M->xfl, (size_t)M->nall) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
     k_excision_flags<<<(unsigned)((M->nall + 255) / 256), 256, 0, st>>>(m, M->xfl, M->nall);
@@ -619,6 +678,7 @@ extern "C" int phx_free_mesh(phx_mesh* M) {
   for (int d = 0; d < 3; ++d) if (M->flux[d]) cudaFree(M->flux[d]);
   if (M->xfl) cudaFree(M->xfl);
   if (M->partial) cudaFree(M->partial);
+  if (M->smax) cudaFree(M->smax);
   for (int d = 0; d < 3; ++d) if (M->ws_field[d]) cudaFree(M->ws_field[d]);
   if (M->ws_mask) cudaFree(M->ws_mask);
   if (M->ws_scal) cudaFree(M->ws_scal);
@@ -740,7 +800,8 @@ static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
 }
 
 static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
-                      const double* d_cons_in, double* d_cons_out, double* d_prim, unsigned char* d_mask, cudaStream_t st) {
+                      const double* d_cons_in, double* d_cons_out, double* d_prim, unsigned char* d_mask, cudaStream_t st,
+                      bool reduce_cfl = false) {
   launch_sweeps(M, d_prim, st);
   { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
   FluxPtrs fl;
@@ -749,8 +810,13 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
   {
   ProfScope ps(M, PHX_K_UPDATE, st);
 #define CALL(MET)                                                                                                                   \
-  if (M->m.excise) k_update<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask); \
-  else k_update<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask)
+  if (M->m.excise) { \
+    if (reduce_cfl) k_update<MET, true, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
+    else k_update<MET, true, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
+  } else { \
+    if (reduce_cfl) k_update<MET, false, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
+    else k_update<MET, false, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
+  }
   DISPATCH_METRIC(M, CALL);
 #undef CALL
   }
@@ -774,6 +840,23 @@ extern "C" int phx_rk2_step(phx_mesh* M, const double* d_dt, double* d_cons0, do
   int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st);
   if (rc != PHX_OK) return rc;
   return stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons, d_cons0, d_cons, d_prim, d_mask, st);
+}
+
+extern "C" int phx_rk2_step_cfl(phx_mesh* M, double cfl, double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
+                                unsigned char* d_mask, void* stream) {
+  if (!M || !d_dt || !(cfl > 0.0) || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask || d_cons0 == d_cons)
+    return fail(PHX_EINVAL, "phx_rk2_step_cfl: null, misaligned or aliased argument, or cfl <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st);
+  if (rc != PHX_OK) return rc;
+  // stage 2 also reduces max sum_d |lambda^d|/dx_d of the new primitives; the final kernel overwrites *d_dt after every
+  // block of stage 2 has read it (stream order)
+  rc = stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons, d_cons0, d_cons, d_prim, d_mask, st, true);
+  if (rc != PHX_OK) return rc;
+  { ProfScope ps(M, PHX_K_CFL, st);
+    k_cfl_final_slots<<<1, 256, 0, st>>>(M->smax, cfl, d_dt); }
+  LAUNCH_CHECK(M, "k_cfl_final_slots");
+  return PHX_OK;
 }
 
 extern "C" int phx_cfl_dt(const phx_mesh* Mc, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream) {
@@ -850,13 +933,15 @@ extern "C" int phx_evolve_host(phx_mesh* M, const double* h_prim_in, int nsteps,
   CUDA_TRY(cudaMemsetAsync(M->ws_mask, 0, (size_t)M->nall, st), "cudaMemsetAsync");
   int rc = phx_prim_to_cons(M, prim, cons, st);
   if (rc != PHX_OK) return rc;
-  for (int s = 0; s < nsteps; ++s) {
+  if (nsteps > 0) {
     rc = phx_cfl_dt(M, prim, cfl, M->ws_scal, nullptr, st);
     if (rc != PHX_OK) return rc;
-    rc = phx_rk2_step(M, M->ws_scal, cons0, cons, prim, M->ws_mask, st);
-    if (rc != PHX_OK) return rc;
-    k_accumulate_time<<<1, 1, 0, st>>>(M->ws_scal);
+  }
+  for (int s = 0; s < nsteps; ++s) {
+    k_accumulate_time<<<1, 1, 0, st>>>(M->ws_scal);      // t += dt of this step, before the step replaces dt
     LAUNCH_CHECK(M, "k_accumulate_time");
+    rc = phx_rk2_step_cfl(M, cfl, M->ws_scal, cons0, cons, prim, M->ws_mask, st);
+    if (rc != PHX_OK) return rc;
   }
   CUDA_TRY(cudaMemcpyAsync(h_prim_out, prim, fbytes, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
   if (h_cons_out) CUDA_TRY(cudaMemcpyAsync(h_cons_out, cons, fbytes, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");

@@ -24,7 +24,7 @@ EXPORTS = (
     "phx_init_mesh", "phx_free_mesh", "phx_field_elems", "phx_mask_elems", "phx_prim_to_cons",
     "phx_cons_to_prim", "phx_fill_ghosts", "phx_rk_stage", "phx_cfl_dt", "phx_rk2_step",
     "phx_evolve_host", "phx_debug_flux", "phx_launch_count", "phx_last_error",
-    "phx_profile_enable", "phx_profile_read",
+    "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl",
 )
 
 
@@ -84,6 +84,7 @@ def lib():
         L.phx_rk_stage.argtypes = [vp, C.c_double, C.c_double, C.c_double, dp, dp, dp, ucp, vp]
         L.phx_cfl_dt.argtypes = [vp, dp, C.c_double, dp, C.POINTER(C.c_double), vp]
         L.phx_rk2_step.argtypes = [vp, dp, dp, dp, dp, ucp, vp]
+        L.phx_rk2_step_cfl.argtypes = [vp, C.c_double, dp, dp, dp, dp, ucp, vp]
         L.phx_evolve_host.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp, vp, C.POINTER(C.c_double), vp]
         L.phx_debug_flux.argtypes = [vp, C.c_int, dp, vp]
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
@@ -203,6 +204,14 @@ def rk2_step(mesh, d_dt, cons0, cons, prim, mask, stream=None):
     _check(lib().phx_rk2_step(mesh.handle, _dev(d_dt, torch.float64, 1, "d_dt"), _dev(cons0, torch.float64, n, "cons0"),
                               _dev(cons, torch.float64, n, "cons"), _dev(prim, torch.float64, n, "prim"),
                               _dev(mask, torch.uint8, mesh.mask_elems, "mask"), _stream(stream)))
+
+
+def rk2_step_cfl(mesh, cfl, d_dt, cons0, cons, prim, mask, stream=None):
+    """RK2 step with dt = d_dt[0], then d_dt[0] <- the CFL time step of the new state (reduction fused into stage 2)."""
+    n = mesh.field_elems
+    _check(lib().phx_rk2_step_cfl(mesh.handle, float(cfl), _dev(d_dt, torch.float64, 1, "d_dt"), _dev(cons0, torch.float64, n, "cons0"),
+                                  _dev(cons, torch.float64, n, "cons"), _dev(prim, torch.float64, n, "prim"),
+                                  _dev(mask, torch.uint8, mesh.mask_elems, "mask"), _stream(stream)))
 
 
 def _host(t, dtype, numel, name, nullable=False):

@@ -63,6 +63,13 @@ class GpuRun:
         self.phx.cfl_dt(self.mesh, self.prim, cfl, self.d_dt)
         self.phx.rk2_step(self.mesh, self.d_dt, self.cons0, self.cons, self.prim, self.mask)
 
+    def step_fused_cfl(self, cfl, first):
+        """The launch configuration bench.py times: phx_rk2_step_cfl (dt of the next step reduced inside stage 2);
+        the first step of a run takes its dt from phx_cfl_dt."""
+        if first:
+            self.phx.cfl_dt(self.mesh, self.prim, cfl, self.d_dt)
+        self.phx.rk2_step_cfl(self.mesh, cfl, self.d_dt, self.cons0, self.cons, self.prim, self.mask)
+
     def dt(self, cfl):
         return self.phx.cfl_dt(self.mesh, self.prim, cfl, self.d_dt, host=True)
 

@@ -1,5 +1,5 @@
 """Full-size GPU parity: BASELINE.json's configs at their full sizes, in the launch configuration bench.py times
-(phx_cfl_dt with the time step kept on the device + phx_rk2_step), checked
+(phx_cfl_dt once, then phx_rk2_step_cfl with the time step kept on the device), checked
 
   (i)  on sampled outputs the oracle can compute one by one: the update of a cell depends on the primitives within
        HALO = 8 cells (two stages x (3 cells of WENO5 stencil to a face + 1 transverse cell of flux-CT)), so the oracle
@@ -86,9 +86,12 @@ def run_full(w, origins, check_conservation):
     c0 = wl.from_blocks(p, g.cons.cpu().numpy())
     div0 = corner_div(c0[5:8], rdx)
     dt_ref = orc.cfl_dt(p, w["prim"], w["cfl"])
-    g.step_device_dt(w["cfl"])                       # phx_cfl_dt (device dt) + phx_rk2_step: what bench.py times
+    g.phx.cfl_dt(g.mesh, g.prim, w["cfl"], g.d_dt)
     dt_gpu = float(g.d_dt.cpu())
     assert abs(dt_gpu - dt_ref) <= 1e-13 * dt_ref
+    g.step_fused_cfl(w["cfl"], first=False)          # phx_rk2_step_cfl with the device dt: what bench.py times
+    dt_next = float(g.d_dt.cpu())
+    assert dt_next == g.dt(w["cfl"])                 # fused reduction = phx_cfl_dt on the new state, bit for bit
     cons, prim, _, mask = g.get()
     assert np.isfinite(cons[:, :, gz:gz + p["nz"], gy:gy + p["ny"], gx:gx + p["nx"]]).all()
     assert not (mask & (16 | 32)).any(), "con2prim failure bits at full size"

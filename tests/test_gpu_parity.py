@@ -231,6 +231,27 @@ def test_device_dt_step_equals_host_dt_step():
     assert np.array_equal(ca, cb) and np.array_equal(pa, pb) and np.array_equal(ma, mb)
 
 
+@pytest.mark.parametrize("name", ["cfg4_turb_24_weno", "cfg5_blocks_2x2x2_of_12", "cfg1_shock_tube_256", "cfg3_ks_torus_28"])
+def test_fused_cfl_step_equals_separate_calls(name):
+    """phx_rk2_step_cfl (what bench.py times) = phx_rk2_step followed by phx_cfl_dt, bit for bit, state and time step;
+    the time step also matches the oracle's CFL time step of the oracle's new state."""
+    w = WORKLOADS[name]
+    p = w["params"]
+    a = GpuRun(p, w["prim"]); b = GpuRun(p, w["prim"])
+    o = orc.Run(p, w["prim"])
+    for n in range(3):
+        a.step_device_dt(0.4)
+        b.step_fused_cfl(0.4, first=(n == 0))
+        o.step(o.dt(0.4))
+        dt_next_a = a.dt(0.4)
+        dt_next_b = float(b.d_dt.cpu())
+        assert dt_next_a == dt_next_b
+        assert abs(dt_next_b - o.dt(0.4)) <= 1e-11 * dt_next_b
+        a.d_dt.fill_(dt_next_a)
+    ca, pa, _, ma = a.get(); cb, pb, _, mb = b.get()
+    assert np.array_equal(ca, cb) and np.array_equal(pa, pb) and np.array_equal(ma, mb)
+
+
 # ----------------------------------------------------------------------------- exact properties on the GPU
 @pytest.mark.parametrize("recon", [0, 1, 2, 3])
 @pytest.mark.parametrize("riemann", [0, 1])
