@@ -59,7 +59,7 @@ NCU_TRAFFIC = {256: {"update": 7.016e9, "sweep_x": 2.207e9, "sweep_y": 2.301e9, 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="zones per side of the config-4 box (256 = BASELINE.json)")
@@ -72,14 +72,14 @@ def parse_args():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
-            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50",
                                        "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
@@ -309,7 +309,7 @@ def run_ours(args):
     if args.workload != "cfg4" or args.n != 256:
         line["roofline"] = None if args.workload != "cfg4" else roofline
     if not args.no_cpu_baseline and world >= 1 and args.workload == "cfg4":
-        ns, steps = 96, 2
+        ns, steps = 128, 3
         zs, per_step = time_oracle(ns, steps)
         line["cpu_baseline"] = {"value": zs * steps / sum(per_step), "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
                                 "sample": f"config-4 recipe at {ns}^3, {steps} RK2 steps ({zs * steps} zone-cycles of the "

@@ -35,7 +35,7 @@ using namespace phx;
 #define PHX_UP_BLOCK 128
 #endif
 #ifndef PHX_UP_MINB
-#define PHX_UP_MINB 6      // Minkowski update: HBM-bound, wants resident warps (80 registers); Kerr-Schild keeps its registers
+#define PHX_UP_MINB 7      // Minkowski update: HBM-bound, wants resident warps (80 registers); Kerr-Schild keeps its registers
 #endif
 #ifndef PHX_UP_MINB_KS
 #define PHX_UP_MINB_KS 4
