@@ -285,6 +285,50 @@ double weno5z_plus(const double f[5]) {
   return (w0 * p0 + w1 * p1 + w2 * p2) / (w0 + w1 + w2);
 }
 
+// WENO5-Z-AOAH (B16-B18).  Nonlinear weights of B14 normalised to sum 1 and the fifth-order value
+// of B12 with those weights, for the +1/2 face of the centre cell of the stencil f[0..4].
+void weno5z_weights(const double f[5], double w[3], double& P5) {
+  const double p0 = (2.0 * f[0] - 7.0 * f[1] + 11.0 * f[2]) / 6.0;
+  const double p1 = (-f[1] + 5.0 * f[2] + 2.0 * f[3]) / 6.0;
+  const double p2 = (2.0 * f[2] + 5.0 * f[3] - f[4]) / 6.0;
+  const double a0 = f[0] - 2.0 * f[1] + f[2], c0 = f[0] - 4.0 * f[1] + 3.0 * f[2];
+  const double a1 = f[1] - 2.0 * f[2] + f[3], c1 = f[1] - f[3];
+  const double a2 = f[2] - 2.0 * f[3] + f[4], c2 = 3.0 * f[2] - 4.0 * f[3] + f[4];
+  const double b0 = 13.0 / 12.0 * a0 * a0 + 0.25 * c0 * c0;
+  const double b1 = 13.0 / 12.0 * a1 * a1 + 0.25 * c1 * c1;
+  const double b2 = 13.0 / 12.0 * a2 * a2 + 0.25 * c2 * c2;
+  const double tau = std::fabs(b2 - b0);
+  const double eps = 1e-40;
+  const double t0 = tau / (b0 + eps), t1 = tau / (b1 + eps), t2 = tau / (b2 + eps);
+  const double u0 = 0.1 * (1.0 + t0 * t0), u1 = 0.6 * (1.0 + t1 * t1), u2 = 0.3 * (1.0 + t2 * t2);
+  const double sum = u0 + u1 + u2;
+  w[0] = u0 / sum; w[1] = u1 / sum; w[2] = u2 / sum;
+  P5 = w[0] * p0 + w[1] * p1 + w[2] * p2;
+}
+// B17: "nonlinearity" of the weights of one face, 1 when w = gamma.
+double aoah_sigma_face(const double w[3]) {
+  const double g0 = 0.1, g1 = 0.6, g2 = 0.3;
+  return 3.0 * w[0] * w[1] * w[2] / (g2 * w[0] * w[1] + g1 * w[0] * w[2] + g0 * w[1] * w[2]);
+}
+// One cell: sigma of B18 from both faces, clamped to [0,1] (B17 can exceed 1, reading C5.1b), then the mix
+// B16 of the WENO5-Z value with the MC-limited piecewise linear value at each face.
+void weno5z_aoah_cell(const double f[5], double& qm, double& qp) {
+  double r[5];
+  for (int m = 0; m < 5; ++m) r[4 - m] = f[m];          // mirror x -> -x
+  double wp[3], wm[3], P5p, P5m;
+  weno5z_weights(f, wp, P5p);
+  weno5z_weights(r, wm, P5m);
+  const double sp = aoah_sigma_face(wp), sm = aoah_sigma_face(wm);
+  double sigma = 2.0 * sp * sm / (sp + sm);
+  if (!(sigma > 0.0)) sigma = 0.0;                        // also catches 0/0 when both faces have a vanishing weight
+  if (sigma > 1.0) sigma = 1.0;
+  const double dl = f[2] - f[1], dr = f[3] - f[2];
+  const double sl = minmod3(2.0 * dl, 0.5 * (f[3] - f[1]), 2.0 * dr);
+  const double plm_p = f[2] + 0.5 * sl, plm_m = f[2] - 0.5 * sl;
+  qp = sigma * P5p + (1.0 - sigma) * plm_p;
+  qm = sigma * P5m + (1.0 - sigma) * plm_m;
+}
+
 // Face values of one variable in one cell from its stencil s[-2..2] (s points at the centre).
 // qm = value at the lower face (x_{j-1/2}, the "R" state of that face), qp = value at the upper
 // face (x_{j+1/2}, the "L" state of that face).
@@ -302,11 +346,12 @@ void recon_cell(int recon, const double* s, long stride, double& qm, double& qp)
   }
   double f[5], r[5];
   for (int m = 0; m < 5; ++m) { f[m] = s[(m - 2) * stride]; r[4 - m] = f[m]; }
+  if (recon == 4) { weno5z_aoah_cell(f, qm, qp); return; }
   qp = weno5z_plus(f);
   qm = weno5z_plus(r);   // mirror x -> -x
 }
 
-int stencil_halfwidth(int recon) { return recon == 0 ? 0 : (recon == 3 ? 2 : 1); }
+int stencil_halfwidth(int recon) { return recon == 0 ? 0 : (recon >= 3 ? 2 : 1); }
 
 // ------------------------------------------------------------------------------------------ C5.2
 void riemann_face(const orc_params& p, const Geo& G, int d, const double qL[NV], const double qR[NV], double F[NV]) {
@@ -578,7 +623,7 @@ void block_fluxes(const Grid& G, int b, const double* prim, std::vector<double> 
           const long c = cid(k, j, i);
           double m[NV], pl[NV];
           for (int v = 0; v < NV; ++v) recon_cell(p.recon, P + v * vstr + c, str[d], m[v], pl[v]);
-          if (p.recon == 3) {
+          if (p.recon >= 3) {
             // positivity fallback: piecewise constant in this direction for all variables
             if (m[RHO] <= p.rho_floor || pl[RHO] <= p.rho_floor || m[UU] <= p.rho_floor * p.eps_floor ||
                 pl[UU] <= p.rho_floor * p.eps_floor)

@@ -585,6 +585,71 @@ def test_p12_reconstruction():
     assert qp[2:-2].max() < 1.0 + 1e-6 and qp[2:-2].min() > -1e-6
 
 
+def test_p12b_weno5z_aoah():
+    """WENO5-Z-AOAH (B16-B18, PAPER.md:820-843)."""
+    AOAH = wl.RECON_WENO5Z_AOAH
+    # B17 with w = gamma gives 1 (PAPER.md:843 "reduces to the standard WENO5-Z method"): on data whose three smoothness
+    # indicators coincide (a parabola: beta_k differ, so take linear data where tau_Z = 0) AOAH = WENO5-Z = exact
+    lin = 2.0 + 0.25 * np.arange(9)
+    qm, qp = orc.recon_line(AOAH, lin)
+    assert np.abs(qp[2:-2] - (lin[2:-2] + 0.125)).max() < 1e-15 and np.abs(qm[2:-2] - (lin[2:-2] - 0.125)).max() < 1e-15
+    # independent derivation: with a_k = 1 + (tau_Z/(beta_k+eps))^2 the harmonic means B17/B18 collapse to
+    # sigma = 15 / [(1/a0 + 1/a1 + 1/a2)(a0 + 3 a1 + a2)]; rebuild the face values from that closed form
+    g = RNG.uniform(size=40) + np.where(np.arange(40) > 20, 3.0, 0.0)
+    qm, qp = orc.recon_line(AOAH, g)
+    wm, wp = orc.recon_line(wl.RECON_WENO5Z, g)
+    mm, mp = orc.recon_line(wl.RECON_PLM_MC, g)
+    for j in range(2, 38):
+        f = g[j - 2: j + 3]
+        b0 = 13 / 12 * (f[0] - 2 * f[1] + f[2]) ** 2 + 0.25 * (f[0] - 4 * f[1] + 3 * f[2]) ** 2
+        b1 = 13 / 12 * (f[1] - 2 * f[2] + f[3]) ** 2 + 0.25 * (f[1] - f[3]) ** 2
+        b2 = 13 / 12 * (f[2] - 2 * f[3] + f[4]) ** 2 + 0.25 * (3 * f[2] - 4 * f[3] + f[4]) ** 2
+        tau = abs(b2 - b0)
+        a = [1 + (tau / (b + 1e-40)) ** 2 for b in (b0, b1, b2)]
+        sig = min(1.0, 15.0 / ((1 / a[0] + 1 / a[1] + 1 / a[2]) * (a[0] + 3 * a[1] + a[2])))
+        assert abs(qp[j] - (sig * wp[j] + (1 - sig) * mp[j])) < 1e-13
+        assert abs(qm[j] - (sig * wm[j] + (1 - sig) * mm[j])) < 1e-13
+        # B16 is a convex combination: the face value lies between the WENO5-Z and the PLM-MC value
+        assert min(wp[j], mp[j]) - 1e-14 <= qp[j] <= max(wp[j], mp[j]) + 1e-14
+    # mirror symmetry
+    qm2, qp2 = orc.recon_line(AOAH, g[::-1].copy())
+    assert np.array_equal(qm[2:-2], qp2[::-1][2:-2])
+    # smooth data: sigma -> 1 fast enough that the fifth order of WENO5-Z survives
+    errs = []
+    for n in (16, 32, 64):
+        h = 1.0 / n
+        xc = (np.arange(-3, n + 3) + 0.5) * h
+        avg = (np.cos(2 * np.pi * (xc - h / 2)) - np.cos(2 * np.pi * (xc + h / 2))) / (2 * np.pi * h)
+        qm, qp = orc.recon_line(AOAH, avg + 2.0)
+        errs.append(np.abs(qp[3:-3] - (np.sin(2 * np.pi * (xc[3:-3] + h / 2)) + 2.0)).max())
+    assert math.log2(errs[0] / errs[1]) > 4.0 and math.log2(errs[1] / errs[2]) > 4.0, errs
+    # at a step the mixing weight collapses: the cells touching the jump get the MC-limited linear value, which has no overshoot at all
+    step = np.where(np.arange(12) < 6, 1.0, 0.0)
+    qm, qp = orc.recon_line(AOAH, step)
+    assert qp[2:-2].max() <= 1.0 + 1e-12 and qp[2:-2].min() >= -1e-12
+    assert qm[2:-2].max() <= 1.0 + 1e-12 and qm[2:-2].min() >= -1e-12
+
+
+def test_p12c_aoah_uniform_and_conservation():
+    """The whole stage with recon = AOAH: uniform state bitwise, totals conserved, corner div B kept."""
+    n = 12
+    p = wl.default_params(nx=n, ny=n, nz=n, ng=4, recon=wl.RECON_WENO5Z_AOAH)
+    q = np.zeros((8, n, n, n))
+    q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7] = 1.3, 0.4, -0.2, 0.1, 2.1, 0.7, -0.3, 0.2
+    o = orc.Run(p, wl.finish(p, q)); c0 = o.cons.copy()
+    o.step(o.dt(0.4))
+    assert np.array_equal(wl.from_blocks(p, o.cons), wl.from_blocks(p, c0))
+    w = wl.turbulence_box(12, recon=wl.RECON_WENO5Z_AOAH)
+    o = orc.Run(w["params"], w["prim"]); c0 = wl.from_blocks(w["params"], o.cons).copy()
+    for _ in range(2):
+        o.step(o.dt(0.4))
+    c1 = wl.from_blocks(w["params"], o.cons)
+    rel = np.abs((c1 - c0).sum(axis=(1, 2, 3))) / np.abs(c0).sum(axis=(1, 2, 3))
+    assert rel.max() < 1e-14, rel
+    d0 = corner_div(c0[5:8], [1.0 / 12] * 3); d1 = corner_div(c1[5:8], [1.0 / 12] * 3)
+    assert np.abs(d1 - d0).max() < 1e-12 * np.abs(c0[5:8]).max() * 12
+
+
 # ----------------------------------------------------------------------------- CFL (C6)
 def test_cfl_closed_form():
     gam = 5.0 / 3.0
