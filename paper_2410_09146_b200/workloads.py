@@ -191,9 +191,9 @@ def solenoidal_from_potential(a0, a1, a2, n):
 
 
 # --------------------------------------------------------------------------- the five configs
-def shock_tube(n=256):
+def shock_tube(n=256, recon=RECON_PLM_MINMOD, ng=2):
     """Config 1: 1-D relativistic MHD shock tube (PAPER.md:443-445 shape; states from BASELINE.json)."""
-    p = default_params(nx=n, ng=2, gamma_ad=2.0, recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL,
+    p = default_params(nx=n, ng=ng, gamma_ad=2.0, recon=recon, riemann=RIEMANN_HLL,
                        bc=((BC_OUTFLOW, BC_OUTFLOW),) * 3, xmin=(0.0, 0.0, 0.0), xmax=(1.0, 1.0, 1.0))
     x = cell_centres(p)[0]
     left = x < 0.5
@@ -250,12 +250,12 @@ def _torus_prims(p, seed):
     return q
 
 
-def kerr_schild_torus(n=128, seed=SEED0 + 3, spin=0.9375, half=20.0):
+def kerr_schild_torus(n=128, seed=SEED0 + 3, spin=0.9375, half=20.0, recon=RECON_PLM_MINMOD):
     """Config 3: single 3-D block in Cartesian Kerr-Schild coordinates, torus-like data."""
     p = default_params(metric=KERR_SCHILD, bh_mass=1.0, bh_spin=spin, r_excise=2.0,
                        nx=n, ny=n, nz=n, ng=4, xmin=(-half,) * 3, xmax=(half,) * 3,
                        bc=((BC_OUTFLOW, BC_OUTFLOW),) * 3, gamma_ad=4.0 / 3.0,
-                       recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL,
+                       recon=recon, riemann=RIEMANN_HLL,
                        rho_floor=1e-6, eps_floor=1e-6, w_max=10.0)
     q = _torus_prims(p, seed)
     return dict(name="cfg3_kerr_schild_torus", params=p, prim=finish(p, q), cfl=0.4, steps=50)

@@ -31,6 +31,10 @@ def small_workloads():
     out["cfg4_turb_24_weno"] = wl.turbulence_box(24)
     out["cfg5_blocks_2x2x2_of_12"] = wl.packed_blocks((2, 2, 2), 12)
     out["cfg5_blocks_3x2x1_of_8"] = wl.packed_blocks((3, 2, 1), 8)
+    # the paper's WENO5-Z-AOAH (App.B B16-B18) on smooth turbulence and on the shock tube
+    out["next1_turb_24_aoah"] = wl.turbulence_box(24, recon=wl.RECON_WENO5Z_AOAH)
+    out["next1_shock_tube_200_aoah"] = wl.shock_tube(200, recon=wl.RECON_WENO5Z_AOAH, ng=3)
+    out["next1_ks_torus_20_aoah"] = wl.kerr_schild_torus(20, recon=wl.RECON_WENO5Z_AOAH)
     return out
 
 
@@ -173,7 +177,7 @@ def test_one_rk2_step_matches_oracle(name):
     print(name, "1-step err per variable", err)
 
 
-@pytest.mark.parametrize("name", ["cfg2_box_24_mc_llf", "cfg4_turb_24_weno"])
+@pytest.mark.parametrize("name", ["cfg2_box_24_mc_llf", "cfg4_turb_24_weno", "next1_turb_24_aoah"])
 def test_raw_riemann_fluxes_match_oracle_without_ct(name):
     """Face fluxes of one stage (CT off so that the oracle's hook returns the raw Riemann fluxes)."""
     torch, phx = _gpu()
@@ -208,7 +212,8 @@ def test_shock_tube_to_t_end_matches_oracle():
 
 
 @pytest.mark.parametrize("name,nsteps", [("cfg2_box_24_mc_llf", 100), ("cfg4_turb_24_weno", 20), ("cfg3_ks_torus_28", 50),
-                                         ("cfg5_blocks_2x2x2_of_12", 20)])
+                                         ("cfg5_blocks_2x2x2_of_12", 20), ("next1_turb_24_aoah", 20),
+                                         ("next1_shock_tube_200_aoah", 100)])
 def test_many_steps_match_oracle(name, nsteps):
     w = WORKLOADS[name]
     p = w["params"]
@@ -253,7 +258,7 @@ def test_fused_cfl_step_equals_separate_calls(name):
 
 
 # ----------------------------------------------------------------------------- exact properties on the GPU
-@pytest.mark.parametrize("recon", [0, 1, 2, 3])
+@pytest.mark.parametrize("recon", [0, 1, 2, 3, 4])
 @pytest.mark.parametrize("riemann", [0, 1])
 def test_uniform_state_stays_bitwise_uniform_on_gpu(recon, riemann):
     n = 20
