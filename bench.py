@@ -63,7 +63,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="zones per side of the config-4 box (256 = BASELINE.json)")
-    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5"],
+    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "next1", "next2"],
                     help="cfg4 (default) is the bench workload; the others time BASELINE.json's other 3-D configs at full size "
                          "(reported without a roofline object: the per-zone figures of DESIGN.md 6 are config 4's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -191,6 +191,12 @@ def run_ours(args):
     if args.workload == "cfg4":
         w = wl.turbulence_box(args.n)
         wname = f"cfg4_turbulence_box_{args.n}^3_weno5z_hll_ct_rk2_minkowski"
+    elif args.workload == "next1":      # config 4 with the paper's WENO5-Z-AOAH reconstruction
+        w = wl.turbulence_box(args.n, recon=wl.RECON_WENO5Z_AOAH)
+        wname = f"next1_turbulence_box_{args.n}^3_weno5z_aoah_hll_ct_rk2_minkowski"
+    elif args.workload == "next2":      # the paper's scaling workload shape, --n 128 is its size
+        w = wl.sedov_blast(args.n)
+        wname = f"next2_sedov_blast_{args.n}^3_plm_minmod_hll_rk2_minkowski"
     elif args.workload == "cfg2":
         w = wl.periodic_box(64); wname = "cfg2_periodic_box_64^3_plm_mc_llf_ct_rk2_minkowski"
     elif args.workload == "cfg3":

@@ -294,6 +294,24 @@ def packed_blocks(nb=(8, 8, 8), n=32, seed=SEED0 + 5, spin=0.5, half=20.0):
     return dict(name="cfg5_packed_blocks", params=p, prim=finish(p, q), cfl=0.4, steps=20)
 
 
+def sedov_blast(n=128, E=1e-5, r_init=0.1, recon=RECON_PLM_MINMOD):
+    """the paper's Sedov-Taylor blast (E = 1e-5 deposited in all cells with
+    r < r_init = 0.1, rho = 1, p = 1e-7, domain [-1,1]^d) as a uniform 3-D block with B = 0 and Gamma = 5/3 -- the
+    shape of the paper's weak-scaling workload (3-D Sedov, 128^3 per start).  The energy is spread evenly
+    over the cells whose centres lie inside r_init, so that the deposited total is exactly E.  No RNG."""
+    p = default_params(nx=n, ny=n, nz=n, ng=4, gamma_ad=5.0 / 3.0, recon=recon, riemann=RIEMANN_HLL,
+                       bc=((BC_OUTFLOW, BC_OUTFLOW),) * 3, xmin=(-1.0,) * 3, xmax=(1.0,) * 3)
+    x, y, z = cell_centres(p)
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    inside = X * X + Y * Y + Z * Z < r_init * r_init
+    dV = (2.0 / n) ** 3
+    q = np.zeros((NV, n, n, n))
+    q[0] = 1.0
+    q[4] = 1e-7 / (p["gamma_ad"] - 1.0)
+    q[4][inside] += E / (inside.sum() * dV)
+    return dict(name="next2_sedov_blast", params=p, prim=finish(p, q), cfl=0.4, steps=20)
+
+
 def reblock(p, prim_blocks, nb):
     """Same global data on a different block decomposition (for the block-invariance pin)."""
     tot = (p["nbx"] * p["nx"], p["nby"] * p["ny"], p["nbz"] * p["nz"])

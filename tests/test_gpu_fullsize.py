@@ -98,6 +98,7 @@ def run_full(w, origins, check_conservation):
     cg = wl.from_blocks(p, cons)
     mg = wl.from_blocks(p, mask[:, None])[0]
     scale = np.abs(cg).reshape(8, -1).max(axis=1)
+    scale = np.where(scale > 0.0, scale, 1.0)          # B = 0 workloads
     ddiv = np.abs(corner_div(cg[5:8], rdx) - div0).max()
     bscale = np.abs(c0[5:8]).max() * max(rdx)
     assert ddiv <= 1e-13 * bscale, f"corner div B changed by {ddiv} (scale {bscale})"
@@ -157,3 +158,18 @@ def test_cfg5_packed_blocks_512x32_sampled():
     n, s = 256, CORE + 2 * HALO
     run_full(w, [(0, 0, 0), (n - s, n - s, n - s), (112, 112, 112), (16, 48, 80), (150, 100, 120), (176, 16, 208)],
              check_conservation=False)
+
+
+def test_next1_turbulence_256_aoah_sampled():
+    """SURVEY.md 8(f) rank 1 at the bench size: config 4's box with WENO5-Z-AOAH (App.B B16-B18)."""
+    w = wl.turbulence_box(256, recon=wl.RECON_WENO5Z_AOAH)
+    n = 256
+    run_full(w, [(0, 0, 0), (n - HALO - 5, 31, 140), (90, 180, n - 12)], check_conservation=True)
+
+
+def test_next2_sedov_128_sampled():
+    """SURVEY.md 8(f) rank 2 at the paper's size (3-D Sedov, 128^3): the deposit region, the domain
+    corner with its outflow faces, and the quiescent ambient medium."""
+    w = wl.sedov_blast(128)
+    n, s = 128, CORE + 2 * HALO
+    run_full(w, [(48, 48, 48), (0, 0, 0), (n - s, 40, 60), (56, 60, 44)], check_conservation=False)

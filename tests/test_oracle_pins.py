@@ -650,6 +650,37 @@ def test_p12c_aoah_uniform_and_conservation():
     assert np.abs(d1 - d0).max() < 1e-12 * np.abs(c0[5:8]).max() * 12
 
 
+def test_p14_sedov_blast_follows_the_self_similar_solution():
+    """3-D Sedov-Taylor blast (PAPER.md:472-484 set-up, B = 0).  With p_ambient << E/R^3 and
+    v << c the flow is the Newtonian self-similar one: shock radius R(t) = xi_0 (E t^2 / rho)^(1/5), xi_0 = 1.15167 for
+    Gamma = 5/3 (Sedov 1946; Taylor 1950).  Pins the whole hydro stage in a strong-shock regime against a textbook
+    closed form: position of the density peak on an axis and on the diagonal, spherical symmetry, energy conservation
+    while the shock is inside the domain."""
+    n = 32
+    w = wl.sedov_blast(n)
+    p = w["params"]
+    o = orc.Run(p, w["prim"])
+    tau0 = wl.from_blocks(p, o.cons)[4].sum(dtype=np.longdouble)
+    t_end = 30.0
+    while o.t < t_end:
+        o.step(min(o.dt(0.4), t_end - o.t))
+    assert not np.bitwise_or.reduce(o.mask.ravel()), "floors or failures in the Sedov run"
+    rho = wl.from_blocks(p, o.prim)[0]
+    h = 2.0 / n
+    R = 1.15167 * (1e-5 * t_end ** 2) ** 0.2
+    c = n // 2
+    r_axis = (np.argmax(rho[c, c, c:]) + 0.5) * h
+    r_diag = (np.argmax([rho[c + i, c + i, c + i] for i in range(n // 2)]) + 0.5) * h * math.sqrt(3.0)
+    assert abs(r_axis - R) <= 1.0 * h, (r_axis, R)
+    assert abs(r_diag - R) <= 1.0 * h * math.sqrt(3.0), (r_diag, R)
+    # octant symmetry of the Cartesian scheme is exact up to round-off; the three axes agree bitwise-ish
+    assert np.abs(rho - rho[::-1, :, :]).max() < 1e-10 and np.abs(rho - rho.transpose(2, 1, 0)).max() < 1e-10
+    # shocked shell is compressed, the interior evacuated, the ambient untouched
+    assert rho.max() > 1.5 and rho[c, c, c] < 0.2 and abs(rho[c, c, -1] - 1.0) < 1e-12
+    tau1 = wl.from_blocks(p, o.cons)[4].sum(dtype=np.longdouble)
+    assert abs(float((tau1 - tau0) / tau0)) < 1e-12
+
+
 # ----------------------------------------------------------------------------- CFL (C6)
 def test_cfl_closed_form():
     gam = 5.0 / 3.0
