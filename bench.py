@@ -63,7 +63,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="zones per side of the config-4 box (256 = BASELINE.json)")
-    ap.add_argument("--workload", default="cfg4", choices=["cfg2", "cfg3", "cfg4", "cfg5", "next1", "next2"],
+    ap.add_argument("--workload", default="cfg4", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "next1", "next2"],
                     help="cfg4 (default) is the bench workload; the others time BASELINE.json's other 3-D configs at full size "
                          "(reported without a roofline object: the per-zone figures of DESIGN.md 6 are config 4's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -130,11 +130,48 @@ def oracle_cores():
         return os.cpu_count() or 1
 
 
-def time_oracle(n, steps):
-    """Zone-cycles/s of the CPU oracle (as it stands, OpenMP over its outer loops) on the config-4 recipe at n^3."""
+def make_workload(name, n):
+    """(workload dict, descriptive name) of a bench workload; n only matters for cfg4 / next1 / next2."""
+    from paper_2410_09146_b200 import workloads as wl
+    if name == "cfg4":
+        return wl.turbulence_box(n), f"cfg4_turbulence_box_{n}^3_weno5z_hll_ct_rk2_minkowski"
+    if name == "next1":     # SURVEY.md 8(f) rank 1: config 4 with the paper's WENO5-Z-AOAH reconstruction
+        return wl.turbulence_box(n, recon=wl.RECON_WENO5Z_AOAH), f"next1_turbulence_box_{n}^3_weno5z_aoah_hll_ct_rk2_minkowski"
+    if name == "next2":     # SURVEY.md 8(f) rank 2: the paper's scaling workload shape (PAPER.md:657), --n 128 is its size
+        return wl.sedov_blast(n), f"next2_sedov_blast_{n}^3_plm_minmod_hll_rk2_minkowski"
+    if name == "cfg1":
+        return wl.shock_tube(256), "cfg1_shock_tube_256_plm_minmod_hll_rk2_minkowski"
+    if name == "cfg2":
+        return wl.periodic_box(64), "cfg2_periodic_box_64^3_plm_mc_llf_ct_rk2_minkowski"
+    if name == "cfg3":
+        return wl.kerr_schild_torus(128), "cfg3_kerr_schild_torus_128^3_plm_minmod_hll_ct_rk2"
+    return wl.packed_blocks((8, 8, 8), 32), "cfg5_packed_blocks_512x32^3_kerr_schild_plm_minmod_hll_ct_rk2"
+
+
+def oracle_sample(name):
+    """Bounded sample of a workload for the oracle's timing: (workload dict, steps, description)."""
+    from paper_2410_09146_b200 import workloads as wl
+    if name == "cfg4":
+        return wl.turbulence_box(128), 3, "config-4 recipe at 128^3, 3 RK2 steps"
+    if name == "next1":
+        return wl.turbulence_box(128, recon=wl.RECON_WENO5Z_AOAH), 3, "config-4 recipe with WENO5-Z-AOAH at 128^3, 3 RK2 steps"
+    if name == "next2":
+        return wl.sedov_blast(128), 3, "Sedov blast at 128^3, 3 RK2 steps"
+    if name == "cfg1":
+        return wl.shock_tube(256), 247, "the whole of config 1 (256 zones, 247 RK2 steps)"
+    if name == "cfg2":
+        return wl.periodic_box(64), 20, "config 2 at full size (64^3), 20 of its 100 RK2 steps"
+    if name == "cfg3":
+        return wl.kerr_schild_torus(96), 3, "config-3 recipe at 96^3, 3 RK2 steps"
+    return wl.packed_blocks((4, 4, 4), 32), 2, "config-5 recipe on 64 blocks of 32^3 (1/8 of the mesh), 2 RK2 steps"
+
+
+def time_oracle(n, steps, w=None):
+    """Zone-cycles/s of the CPU oracle (as it stands, OpenMP over its outer loops); default: config-4 recipe at n^3."""
     from oracle import orc
     from paper_2410_09146_b200 import workloads as wl
-    w = wl.turbulence_box(n)
+    if w is None:
+        w = wl.turbulence_box(n)
     o = orc.Run(w["params"], w["prim"])
     per_step = []
     for _ in range(steps):
@@ -188,21 +225,7 @@ def run_ours(args):
     phx.lib()   # fails loudly if libphx.so is missing
 
     K, W = args.steps, max(args.warmup, 0)
-    if args.workload == "cfg4":
-        w = wl.turbulence_box(args.n)
-        wname = f"cfg4_turbulence_box_{args.n}^3_weno5z_hll_ct_rk2_minkowski"
-    elif args.workload == "next1":      # config 4 with the paper's WENO5-Z-AOAH reconstruction
-        w = wl.turbulence_box(args.n, recon=wl.RECON_WENO5Z_AOAH)
-        wname = f"next1_turbulence_box_{args.n}^3_weno5z_aoah_hll_ct_rk2_minkowski"
-    elif args.workload == "next2":      # the paper's scaling workload shape, --n 128 is its size
-        w = wl.sedov_blast(args.n)
-        wname = f"next2_sedov_blast_{args.n}^3_plm_minmod_hll_rk2_minkowski"
-    elif args.workload == "cfg2":
-        w = wl.periodic_box(64); wname = "cfg2_periodic_box_64^3_plm_mc_llf_ct_rk2_minkowski"
-    elif args.workload == "cfg3":
-        w = wl.kerr_schild_torus(128); wname = "cfg3_kerr_schild_torus_128^3_plm_minmod_hll_ct_rk2"
-    else:
-        w = wl.packed_blocks((8, 8, 8), 32); wname = "cfg5_packed_blocks_512x32^3_kerr_schild_plm_minmod_hll_ct_rk2"
+    w, wname = make_workload(args.workload, args.n)
     p = w["params"]
     zones = wl.n_zones(p)
     mesh = phx.init_mesh(p)
@@ -314,12 +337,11 @@ def run_ours(args):
     }
     if args.workload != "cfg4" or args.n != 256:
         line["roofline"] = None if args.workload != "cfg4" else roofline
-    if not args.no_cpu_baseline and world >= 1 and args.workload == "cfg4":
-        ns, steps = 128, 3
-        zs, per_step = time_oracle(ns, steps)
+    if not args.no_cpu_baseline and world >= 1:
+        ws, steps, what = oracle_sample(args.workload)
+        zs, per_step = time_oracle(0, steps, ws)
         line["cpu_baseline"] = {"value": zs * steps / sum(per_step), "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
-                                "sample": f"config-4 recipe at {ns}^3, {steps} RK2 steps ({zs * steps} zone-cycles of the "
-                                          f"{zones * K} timed on the GPU)"}
+                                "sample": f"{what} ({zs * steps} zone-cycles; {zones * K} timed on the GPU)"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
