@@ -329,6 +329,33 @@ void weno5z_aoah_cell(const double f[5], double& qm, double& qp) {
   qm = sigma * P5m + (1.0 - sigma) * plm_m;
 }
 
+// MP5 (Suresh & Huynh 1997; named at PAPER.md:275, no parameters given -> alpha = 4, eps = 1e-10 of the original paper).
+// Value at the +1/2 face of the centre cell of f[0..4]: the fifth-order linear value, kept if it lies between f_j and
+// the monotonicity-preserving bound, else limited to the interval [vmin, vmax] built from the curvature measures d.
+double minmod4(double a, double b, double c, double d) {
+  if (a > 0.0 && b > 0.0 && c > 0.0 && d > 0.0) return std::fmin(std::fmin(a, b), std::fmin(c, d));
+  if (a < 0.0 && b < 0.0 && c < 0.0 && d < 0.0) return std::fmax(std::fmax(a, b), std::fmax(c, d));
+  return 0.0;
+}
+double mp5_plus(const double f[5]) {
+  const double alpha = 4.0, eps = 1e-10;
+  const double vor = (2.0 * f[0] - 13.0 * f[1] + 47.0 * f[2] + 27.0 * f[3] - 3.0 * f[4]) / 60.0;
+  const double vmp = f[2] + minmod2(f[3] - f[2], alpha * (f[2] - f[1]));
+  if ((vor - f[2]) * (vor - vmp) <= eps) return vor;
+  const double djm1 = f[0] - 2.0 * f[1] + f[2];
+  const double dj = f[1] - 2.0 * f[2] + f[3];
+  const double djp1 = f[2] - 2.0 * f[3] + f[4];
+  const double dm4jph = minmod4(4.0 * dj - djp1, 4.0 * djp1 - dj, dj, djp1);
+  const double dm4jmh = minmod4(4.0 * dj - djm1, 4.0 * djm1 - dj, dj, djm1);
+  const double vul = f[2] + alpha * (f[2] - f[1]);
+  const double vav = 0.5 * (f[2] + f[3]);
+  const double vmd = vav - 0.5 * dm4jph;
+  const double vlc = f[2] + 0.5 * (f[2] - f[1]) + 4.0 / 3.0 * dm4jmh;
+  const double vmin = std::fmax(std::fmin(std::fmin(f[2], f[3]), vmd), std::fmin(std::fmin(f[2], vul), vlc));
+  const double vmax = std::fmin(std::fmax(std::fmax(f[2], f[3]), vmd), std::fmax(std::fmax(f[2], vul), vlc));
+  return vor + minmod2(vmin - vor, vmax - vor);
+}
+
 // Face values of one variable in one cell from its stencil s[-2..2] (s points at the centre).
 // qm = value at the lower face (x_{j-1/2}, the "R" state of that face), qp = value at the upper
 // face (x_{j+1/2}, the "L" state of that face).
@@ -347,6 +374,7 @@ void recon_cell(int recon, const double* s, long stride, double& qm, double& qp)
   double f[5], r[5];
   for (int m = 0; m < 5; ++m) { f[m] = s[(m - 2) * stride]; r[4 - m] = f[m]; }
   if (recon == 4) { weno5z_aoah_cell(f, qm, qp); return; }
+  if (recon == 5) { qp = mp5_plus(f); qm = mp5_plus(r); return; }
   qp = weno5z_plus(f);
   qm = weno5z_plus(r);   // mirror x -> -x
 }

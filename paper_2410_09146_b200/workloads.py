@@ -21,7 +21,7 @@ NV = 8
 SEED0 = 241009146
 
 MINKOWSKI, KERR_SCHILD = 0, 1
-RECON_CONST, RECON_PLM_MINMOD, RECON_PLM_MC, RECON_WENO5Z, RECON_WENO5Z_AOAH = 0, 1, 2, 3, 4
+RECON_CONST, RECON_PLM_MINMOD, RECON_PLM_MC, RECON_WENO5Z, RECON_WENO5Z_AOAH, RECON_MP5 = 0, 1, 2, 3, 4, 5
 RIEMANN_LLF, RIEMANN_HLL = 0, 1
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 

@@ -630,6 +630,51 @@ def test_p12b_weno5z_aoah():
     assert qm[2:-2].max() <= 1.0 + 1e-12 and qm[2:-2].min() >= -1e-12
 
 
+def test_p12d_mp5():
+    """MP5 (Suresh & Huynh 1997)."""
+    MP5 = wl.RECON_MP5
+    # hand-worked: stencil (0,0,0,1,1): linear value 24/60 = 0.4 violates the bound v_mp = f_j = 0; the curvature
+    # measures d = (0, 1, -1) give d^M4 = 0 on both sides, v_UL = v_LC = 0, v_MD = 1/2 -> [vmin, vmax] = [0, 0] -> 0.
+    qm, qp = orc.recon_line(MP5, np.array([0.0, 0.0, 0.0, 1.0, 1.0]))
+    assert qp[2] == 0.0
+    # the mirrored face of the same cell: stencil (1,1,0,0,0) -> v_or = (2-13)/60 < 0 = f_j = v_mp -> product > 0 -> limited to 0
+    assert qm[2] == 0.0
+    # smooth monotone stencil: the unlimited value (2,-13,47,27,-3)/60
+    f = np.array([1.0, 1.5, 2.1, 2.8, 3.6])
+    qm, qp = orc.recon_line(MP5, f)
+    assert abs(qp[2] - (2 * 1.0 - 13 * 1.5 + 47 * 2.1 + 27 * 2.8 - 3 * 3.6) / 60.0) < 1e-15
+    # linear data exact, mirror symmetry
+    lin = 2.0 + 0.25 * np.arange(9)
+    qm, qp = orc.recon_line(MP5, lin)
+    assert np.abs(qp[2:-2] - (lin[2:-2] + 0.125)).max() < 1e-15 and np.abs(qm[2:-2] - (lin[2:-2] - 0.125)).max() < 1e-15
+    g = RNG.uniform(size=30)
+    qm1, qp1 = orc.recon_line(MP5, g)
+    qm2, qp2 = orc.recon_line(MP5, g[::-1].copy())
+    assert np.array_equal(qm1[2:-2], qp2[::-1][2:-2])
+    # fifth order on smooth cell averages, extrema included (alpha = 4 leaves them alone)
+    errs = []
+    for n in (16, 32, 64):
+        h = 1.0 / n
+        xc = (np.arange(-3, n + 3) + 0.5) * h
+        avg = (np.cos(2 * np.pi * (xc - h / 2)) - np.cos(2 * np.pi * (xc + h / 2))) / (2 * np.pi * h)
+        qm, qp = orc.recon_line(MP5, avg + 2.0)
+        errs.append(np.abs(qp[3:-3] - (np.sin(2 * np.pi * (xc[3:-3] + h / 2)) + 2.0)).max())
+    assert math.log2(errs[0] / errs[1]) > 4.5 and math.log2(errs[1] / errs[2]) > 4.5, errs
+    # monotonicity preservation: on monotone data every face value lies between the two adjacent cell values
+    mono = np.cumsum(RNG.uniform(size=40) ** 4)
+    qm, qp = orc.recon_line(MP5, mono)
+    assert np.all(qp[2:-2] >= mono[2:-2] - 1e-14) and np.all(qp[2:-2] <= mono[3:-1] + 1e-14)
+    assert np.all(qm[2:-2] <= mono[2:-2] + 1e-14) and np.all(qm[2:-2] >= mono[1:-3] - 1e-14)
+    # whole stage: uniform state bitwise
+    n = 10
+    p = wl.default_params(nx=n, ny=n, nz=n, ng=3, recon=MP5)
+    q = np.zeros((8, n, n, n))
+    q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7] = 1.3, 0.4, -0.2, 0.1, 2.1, 0.7, -0.3, 0.2
+    o = orc.Run(p, wl.finish(p, q)); c0 = o.cons.copy()
+    o.step(o.dt(0.4))
+    assert np.array_equal(wl.from_blocks(p, o.cons), wl.from_blocks(p, c0))
+
+
 def test_p12c_aoah_uniform_and_conservation():
     """The whole stage with recon = AOAH: uniform state bitwise, totals conserved, corner div B kept."""
     n = 12
