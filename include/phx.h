@@ -27,7 +27,8 @@ typedef struct phx_mesh phx_mesh; /* opaque; owns flux scratch, excision flags a
 enum { PHX_OK = 0, PHX_EINVAL = 1, PHX_ECUDA = 2, PHX_ENOMEM = 3, PHX_EUNSUPPORTED = 4 };
 enum { PHX_MINKOWSKI = 0, PHX_KERR_SCHILD = 1 }; /* Cartesian Kerr-Schild, ingoing (analytic metrics) */
 enum { PHX_RECON_CONST = 0, PHX_RECON_PLM_MINMOD = 1, PHX_RECON_PLM_MC = 2, PHX_RECON_WENO5Z = 3,    /* PAPER.md:275, App.B B12-B15 */
-       PHX_RECON_WENO5Z_AOAH = 4 };  /* the paper's WENO5-Z mixed with PLM-MC by the weight sigma, App.B B16-B18 */
+       PHX_RECON_WENO5Z_AOAH = 4,    /* the paper's WENO5-Z mixed with PLM-MC by the weight sigma, App.B B16-B18 */
+       PHX_RECON_MP5 = 5 };          /* Suresh & Huynh (1997) monotonicity-preserving fifth order, alpha = 4 */
 enum { PHX_RIEMANN_LLF = 0, PHX_RIEMANN_HLL = 1 };
 enum { PHX_BC_PERIODIC = 0, PHX_BC_OUTFLOW = 1 };
 /* con2prim / floor mask bits */
@@ -41,7 +42,7 @@ typedef struct {
   double bh_mass, bh_spin, r_excise; /* Kerr-Schild only; r_excise <= 0: no excision */
   int nbx, nby, nbz;                 /* block grid */
   int nx, ny, nz;                    /* interior zones per block */
-  int ng;                            /* ghosts per side in active dimensions: >=2 for PLM, >=3 for WENO5-Z(-AOAH) */
+  int ng;                            /* ghosts per side in active dimensions: >=2 for PLM, >=3 for WENO5-Z(-AOAH) and MP5 */
   double xmin[3], xmax[3];           /* global domain, uniform spacing */
   int bc[3][2];                      /* [dimension][lower, upper] */
   double gamma_ad;                   /* ideal gas P = (Gamma-1) rho eps */

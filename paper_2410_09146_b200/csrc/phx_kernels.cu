@@ -602,7 +602,7 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   *out = nullptr;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->nbx < 1 || p->nby < 1 || p->nbz < 1) return fail(PHX_EINVAL, "phx_init_mesh: sizes must be >= 1");
   if (p->metric != PHX_MINKOWSKI && p->metric != PHX_KERR_SCHILD) return fail(PHX_EINVAL, "phx_init_mesh: unknown metric");
-  if (p->recon < 0 || p->recon > 4) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown reconstruction");
+  if (p->recon < 0 || p->recon > 5) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown reconstruction");
   if (p->riemann < 0 || p->riemann > 1) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown Riemann solver");
   const int need = (p->recon >= 3) ? 3 : 2;
   if (p->ng < need) return fail(PHX_EINVAL, "phx_init_mesh: ng too small for the reconstruction stencil (>=2 PLM, >=3 WENO5-Z)");
@@ -786,18 +786,20 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
 }
 
 static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
-  const int key = M->m.metric * 5 + M->m.recon;
+  const int key = M->m.metric * 6 + M->m.recon;
   switch (key) {
     case 0: launch_sweeps_t<0, 0>(M, prim, st); break;
     case 1: launch_sweeps_t<0, 1>(M, prim, st); break;
     case 2: launch_sweeps_t<0, 2>(M, prim, st); break;
     case 3: launch_sweeps_t<0, 3>(M, prim, st); break;
     case 4: launch_sweeps_t<0, 4>(M, prim, st); break;
-    case 5: launch_sweeps_t<1, 0>(M, prim, st); break;
-    case 6: launch_sweeps_t<1, 1>(M, prim, st); break;
-    case 7: launch_sweeps_t<1, 2>(M, prim, st); break;
-    case 8: launch_sweeps_t<1, 3>(M, prim, st); break;
-    default: launch_sweeps_t<1, 4>(M, prim, st); break;
+    case 5: launch_sweeps_t<0, 5>(M, prim, st); break;
+    case 6: launch_sweeps_t<1, 0>(M, prim, st); break;
+    case 7: launch_sweeps_t<1, 1>(M, prim, st); break;
+    case 8: launch_sweeps_t<1, 2>(M, prim, st); break;
+    case 9: launch_sweeps_t<1, 3>(M, prim, st); break;
+    case 10: launch_sweeps_t<1, 4>(M, prim, st); break;
+    default: launch_sweeps_t<1, 5>(M, prim, st); break;
   }
 }
 

@@ -35,6 +35,8 @@ def small_workloads():
     out["next1_turb_24_aoah"] = wl.turbulence_box(24, recon=wl.RECON_WENO5Z_AOAH)
     out["next1_shock_tube_200_aoah"] = wl.shock_tube(200, recon=wl.RECON_WENO5Z_AOAH, ng=3)
     out["next1_ks_torus_20_aoah"] = wl.kerr_schild_torus(20, recon=wl.RECON_WENO5Z_AOAH)
+    out["next1b_turb_20_mp5"] = wl.turbulence_box(20, recon=wl.RECON_MP5)
+    out["next1b_shock_tube_200_mp5"] = wl.shock_tube(200, recon=wl.RECON_MP5, ng=3)
     # 3-D Sedov-Taylor blast, B = 0 (the paper's scaling workload shape)
     out["next2_sedov_24"] = wl.sedov_blast(24)
     out["next2_sedov_20_aoah"] = wl.sedov_blast(20, recon=wl.RECON_WENO5Z_AOAH)
@@ -216,7 +218,7 @@ def test_shock_tube_to_t_end_matches_oracle():
 
 @pytest.mark.parametrize("name,nsteps", [("cfg2_box_24_mc_llf", 100), ("cfg4_turb_24_weno", 20), ("cfg3_ks_torus_28", 50),
                                          ("cfg5_blocks_2x2x2_of_12", 20), ("next1_turb_24_aoah", 20),
-                                         ("next1_shock_tube_200_aoah", 100), ("next2_sedov_24", 60),
+                                         ("next1_shock_tube_200_aoah", 100), ("next2_sedov_24", 60), ("next1b_turb_20_mp5", 20), ("next1b_shock_tube_200_mp5", 100),
                                          ("next2_sedov_20_aoah", 40)])
 def test_many_steps_match_oracle(name, nsteps):
     w = WORKLOADS[name]
@@ -262,7 +264,7 @@ def test_fused_cfl_step_equals_separate_calls(name):
 
 
 # ----------------------------------------------------------------------------- exact properties on the GPU
-@pytest.mark.parametrize("recon", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("recon", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("riemann", [0, 1])
 def test_uniform_state_stays_bitwise_uniform_on_gpu(recon, riemann):
     n = 20
