@@ -207,6 +207,18 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def aggregate(ms_local, zones, steps, world, device):
+    """Whole-job figure of `world` independent replicas (replicas only, no data-path collective): the device
+    time is the MAX over ranks, value = world x zones x steps / that time.  Returns (ms, zone-cycles/s)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    return ms, world * zones * steps / (ms * 1e-3)
+
+
 # --------------------------------------------------------------------------------------------- the CUDA path
 def run_ours(args):
     import numpy as np
@@ -267,11 +279,7 @@ def run_ours(args):
     mesh.profile_enable(0)
     bad = int(mask.to(torch.int32).bitwise_and(16 | 32).count_nonzero().item())   # no-convergence / bad-input cells
     finite = bool(torch.isfinite(cons).all().item())
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * zones * K / (ms * 1e-3)
+    ms, value = aggregate(ms, zones, K, world, "cuda")
 
     # ---- end to end through the HOST-buffer C-ABI call (rank-local replica; max over ranks)
     e2e = None
@@ -289,10 +297,8 @@ def run_ours(args):
             phx.evolve_host(mesh, hin, 1, w["cfl"], hp, hc, hm)
         e1.record()
         barrier()
-        t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * zones * ke / (float(t.item()) * 1e-3), "unit": UNIT,
+        _, e2e_value = aggregate(e0.elapsed_time(e1), zones, ke, world, "cuda")
+        e2e = {"value": e2e_value, "unit": UNIT,
                "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": 2 * field_bytes + hm.numel() + 16,
                "steps": ke, "call": "phx_evolve_host(nsteps=1) per step, pinned host buffers"}
     if rank != 0:
