@@ -25,7 +25,9 @@ extern "C" {
 typedef struct phx_mesh phx_mesh; /* opaque; owns flux scratch, excision flags and reduction scratch on the device */
 
 enum { PHX_OK = 0, PHX_EINVAL = 1, PHX_ECUDA = 2, PHX_ENOMEM = 3, PHX_EUNSUPPORTED = 4 };
-enum { PHX_MINKOWSKI = 0, PHX_KERR_SCHILD = 1 }; /* Cartesian Kerr-Schild, ingoing (analytic metrics) */
+enum { PHX_MINKOWSKI = 0, PHX_KERR_SCHILD = 1,   /* Cartesian Kerr-Schild, ingoing (analytic metrics) */
+       PHX_MINKOWSKI_BOOSTED = 2 };              /* flat metric in coordinates x' = x - shift*t: alpha = 1, beta^i = shift^i,
+                                                    gamma_ij = delta_ij ("flat metric with coordinate boosts") */
 enum { PHX_RECON_CONST = 0, PHX_RECON_PLM_MINMOD = 1, PHX_RECON_PLM_MC = 2, PHX_RECON_WENO5Z = 3,    /* PAPER.md:275, App.B B12-B15 */
        PHX_RECON_WENO5Z_AOAH = 4,    /* the paper's WENO5-Z mixed with PLM-MC by the weight sigma, App.B B16-B18 */
        PHX_RECON_MP5 = 5 };          /* Suresh & Huynh (1997) monotonicity-preserving fifth order, alpha = 4 */
@@ -50,6 +52,7 @@ typedef struct {
   double rho_floor, eps_floor, w_max; /* constant-form floors (first case) */
   double c2p_tol;                     /* relative tolerance on the con2prim root mu */
   int c2p_maxit;
+  double shift[3];                    /* PHX_MINKOWSKI_BOOSTED only: the constant shift vector, |shift| < 1 */
 } phx_params;
 
 /* Build a mesh object: validates the parameters, allocates flux scratch (3 x one 8-variable field),

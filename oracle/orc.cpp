@@ -40,6 +40,7 @@ typedef struct {
   double gamma_ad;  int recon, riemann, use_ct;
   double rho_floor, eps_floor, w_max;
   double c2p_tol;  int c2p_maxit;
+  double shift[3];   /* metric 2: flat metric in coordinates boosted by x' = x - shift*t */
 } orc_params;
 }
 
@@ -117,6 +118,13 @@ void metric4(const orc_params& p, const double x[3], double g[4][4]) {
     double r, H, l[4];
     ks_scalars(p, x, r, H, l);
     for (int m = 0; m < 4; ++m) for (int n = 0; n < 4; ++n) g[m][n] += 2.0 * H * l[m] * l[n];
+  }
+  if (p.metric == 2) {
+    // "flat metric with coordinate boosts" (reading C2b): x = x' + v t turns
+    // ds^2 = -dt^2 + dx^2 into -(1 - v^2) dt^2 + 2 v_i dx'^i dt + dx'^2, i.e. alpha = 1, beta^i = v^i, gamma_ij = delta_ij
+    double v2 = 0.0;
+    for (int i = 0; i < 3; ++i) { g[0][i + 1] = g[i + 1][0] = p.shift[i]; v2 += p.shift[i] * p.shift[i]; }
+    g[0][0] = -1.0 + v2;
   }
 }
 

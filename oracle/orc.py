@@ -25,15 +25,18 @@ class Params(C.Structure):
         ("xmin", C.c_double * 3), ("xmax", C.c_double * 3), ("bc", (C.c_int * 2) * 3),
         ("gamma_ad", C.c_double), ("recon", C.c_int), ("riemann", C.c_int), ("use_ct", C.c_int),
         ("rho_floor", C.c_double), ("eps_floor", C.c_double), ("w_max", C.c_double),
-        ("c2p_tol", C.c_double), ("c2p_maxit", C.c_int),
+        ("c2p_tol", C.c_double), ("c2p_maxit", C.c_int), ("shift", C.c_double * 3),
     ]
 
 
 def make_params(p: dict) -> Params:
     q = Params()
     for name, _ in Params._fields_:
-        v = p[name]
-        if name in ("xmin", "xmax"):
+        if name == "shift":
+            v = p.get("shift", (0.0, 0.0, 0.0))
+        else:
+            v = p[name]
+        if name in ("xmin", "xmax", "shift"):
             setattr(q, name, (C.c_double * 3)(*v))
         elif name == "bc":
             arr = ((C.c_int * 2) * 3)()

@@ -331,7 +331,7 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
 // orders like the unsigned integer), one atomicMax per thread block; k_cfl_final_slots turns them into the time step.
 constexpr int PHX_NSLOT = 1024;
 template <int METRIC, bool EXC, bool CFL>
-__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 0 ? PHX_UP_MINB : PHX_UP_MINB_KS)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
+__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 1 ? PHX_UP_MINB_KS : PHX_UP_MINB)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                                      double bdt_host, const double* __restrict__ d_dt, double beta,
                                                      const double* cons0, const double* cons_in, double* cons_out,
                                                      double* __restrict__ prim, unsigned char* __restrict__ mask,
@@ -601,7 +601,9 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   if (!p || !out) return fail(PHX_EINVAL, "phx_init_mesh: null argument");
   *out = nullptr;
   if (p->nx < 1 || p->ny < 1 || p->nz < 1 || p->nbx < 1 || p->nby < 1 || p->nbz < 1) return fail(PHX_EINVAL, "phx_init_mesh: sizes must be >= 1");
-  if (p->metric != PHX_MINKOWSKI && p->metric != PHX_KERR_SCHILD) return fail(PHX_EINVAL, "phx_init_mesh: unknown metric");
+  if (p->metric != PHX_MINKOWSKI && p->metric != PHX_KERR_SCHILD && p->metric != PHX_MINKOWSKI_BOOSTED) return fail(PHX_EINVAL, "phx_init_mesh: unknown metric");
+  if (p->metric == PHX_MINKOWSKI_BOOSTED && !(p->shift[0] * p->shift[0] + p->shift[1] * p->shift[1] + p->shift[2] * p->shift[2] < 1.0))
+    return fail(PHX_EINVAL, "phx_init_mesh: |shift| must be below 1");
   if (p->recon < 0 || p->recon > 5) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown reconstruction");
   if (p->riemann < 0 || p->riemann > 1) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown Riemann solver");
   const int need = (p->recon >= 3) ? 3 : 2;
@@ -641,6 +643,7 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   m.gam = p->gamma_ad; m.recon = p->recon; m.riemann = p->riemann; m.use_ct = p->use_ct ? 1 : 0;
   m.rho_floor = p->rho_floor; m.eps_floor = p->eps_floor; m.w_max = p->w_max; m.c2p_tol = p->c2p_tol; m.c2p_maxit = p->c2p_maxit;
   m.excise = (p->metric == PHX_KERR_SCHILD && p->r_excise > 0.0) ? 1 : 0;
+  for (int d = 0; d < 3; ++d) m.shift[d] = (p->metric == PHX_MINKOWSKI_BOOSTED) ? p->shift[d] : 0.0;
   M->nall = (long long)m.nblk * m.ncell;
   M->ninterior = (long long)m.nblk * m.n[0] * m.n[1] * m.n[2];
   if (M->nall * NV >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
@@ -699,7 +702,8 @@ extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* str
 #define DISPATCH_METRIC(mesh, CALL)                 \
   do {                                              \
     if ((mesh)->m.metric == 0) { CALL(0); }         \
-    else { CALL(1); }                               \
+    else if ((mesh)->m.metric == 1) { CALL(1); }    \
+    else { CALL(2); }                               \
   } while (0)
 
 extern "C" int phx_prim_to_cons(const phx_mesh* Mc, const double* d_prim, double* d_cons, void* stream) {
@@ -788,18 +792,12 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
 static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
   const int key = M->m.metric * 6 + M->m.recon;
   switch (key) {
-    case 0: launch_sweeps_t<0, 0>(M, prim, st); break;
-    case 1: launch_sweeps_t<0, 1>(M, prim, st); break;
-    case 2: launch_sweeps_t<0, 2>(M, prim, st); break;
-    case 3: launch_sweeps_t<0, 3>(M, prim, st); break;
-    case 4: launch_sweeps_t<0, 4>(M, prim, st); break;
-    case 5: launch_sweeps_t<0, 5>(M, prim, st); break;
-    case 6: launch_sweeps_t<1, 0>(M, prim, st); break;
-    case 7: launch_sweeps_t<1, 1>(M, prim, st); break;
-    case 8: launch_sweeps_t<1, 2>(M, prim, st); break;
-    case 9: launch_sweeps_t<1, 3>(M, prim, st); break;
-    case 10: launch_sweeps_t<1, 4>(M, prim, st); break;
-    default: launch_sweeps_t<1, 5>(M, prim, st); break;
+#define PHX_CASE(MET, REC) case MET * 6 + REC: launch_sweeps_t<MET, REC>(M, prim, st); break;
+    PHX_CASE(0, 0) PHX_CASE(0, 1) PHX_CASE(0, 2) PHX_CASE(0, 3) PHX_CASE(0, 4) PHX_CASE(0, 5)
+    PHX_CASE(1, 0) PHX_CASE(1, 1) PHX_CASE(1, 2) PHX_CASE(1, 3) PHX_CASE(1, 4) PHX_CASE(1, 5)
+    PHX_CASE(2, 0) PHX_CASE(2, 1) PHX_CASE(2, 2) PHX_CASE(2, 3) PHX_CASE(2, 4) PHX_CASE(2, 5)
+#undef PHX_CASE
+    default: break;
   }
 }
 

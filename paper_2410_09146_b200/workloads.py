@@ -20,7 +20,7 @@ import numpy as np
 NV = 8
 SEED0 = 241009146
 
-MINKOWSKI, KERR_SCHILD = 0, 1
+MINKOWSKI, KERR_SCHILD, MINKOWSKI_BOOSTED = 0, 1, 2
 RECON_CONST, RECON_PLM_MINMOD, RECON_PLM_MC, RECON_WENO5Z, RECON_WENO5Z_AOAH, RECON_MP5 = 0, 1, 2, 3, 4, 5
 RIEMANN_LLF, RIEMANN_HLL = 0, 1
 BC_PERIODIC, BC_OUTFLOW = 0, 1
@@ -34,6 +34,7 @@ def default_params(**kw):
         bc=((BC_PERIODIC, BC_PERIODIC),) * 3,
         gamma_ad=5.0 / 3.0, recon=RECON_PLM_MINMOD, riemann=RIEMANN_HLL, use_ct=1,
         rho_floor=1e-10, eps_floor=1e-10, w_max=50.0, c2p_tol=1e-15, c2p_maxit=64,
+        shift=(0.0, 0.0, 0.0),
     )
     p.update(kw)
     return p
@@ -310,6 +311,45 @@ def sedov_blast(n=128, E=1e-5, r_init=0.1, recon=RECON_PLM_MINMOD):
     q[4] = 1e-7 / (p["gamma_ad"] - 1.0)
     q[4][inside] += E / (inside.sum() * dV)
     return dict(name="next2_sedov_blast", params=p, prim=finish(p, q), cfl=0.4, steps=20)
+
+
+def boosted_linear_wave(n=64, kind="sound", boost=0.617213, A=1e-6, recon=RECON_PLM_MC):
+    """the paper's linear-wave set-up: 2-D, Gamma = 5/3, flat metric with
+    coordinate boosts v_x = v_y = 0.617213, periodic unit square.  Background rho = P = 1 at rest in the unboosted frame;
+    a plane wave of amplitude A with phase 2 pi (x + y) travelling against the boost (so that one period of the pattern in
+    the boosted coordinates is short): sound (drho = A rho, dP = A rho h c_s^2, dv = -A c_s n) or Alfven with B_0 = 1 along
+    n = (1,1)/sqrt 2 (dv_z = A, dB_z = +A sqrt(rho h + B_0^2)).  Returns the workload plus the period T of the pattern
+    and the index of the variable the L1 norm of Eq.61 is taken of.  No RNG."""
+    gam = 5.0 / 3.0
+    p = default_params(metric=MINKOWSKI_BOOSTED, shift=(boost, boost, 0.0), nx=n, ny=n, nz=1, ng=2 if recon in (1, 2) else 3,
+                       gamma_ad=gam, recon=recon, riemann=RIEMANN_HLL)
+    x, y, _ = cell_centres(p)
+    Y, X = np.meshgrid(y, x, indexing="ij")
+    s = np.sin(2.0 * np.pi * (X + Y))[None]           # [1, Ny, Nx]
+    rho0, P0, B0 = 1.0, 1.0, 1.0
+    rhoh = rho0 + P0 / (gam - 1.0) + P0
+    q = np.zeros((NV, 1, n, n))
+    q[0], q[4] = rho0, P0 / (gam - 1.0)
+    r2 = np.sqrt(0.5)
+    if kind == "sound":
+        cs = np.sqrt(gam * P0 / rhoh)
+        q[0] += A * rho0 * s
+        q[4] += A * rhoh * cs * cs * s / (gam - 1.0)
+        v = -A * cs * s
+        W = 1.0 / np.sqrt(1.0 - v * v)
+        q[1], q[2] = W * v * r2, W * v * r2
+        lam, var = cs, 0
+    elif kind == "alfven":
+        q[5], q[6] = B0 * r2, B0 * r2
+        lam = B0 / np.sqrt(rhoh + B0 * B0)
+        v = A * s
+        q[3] = v / np.sqrt(1.0 - v * v)
+        q[7] = A * np.sqrt(rhoh + B0 * B0) * s
+        var = 7
+    else:
+        raise ValueError(kind)
+    T = 1.0 / (np.sqrt(2.0) * lam + 2.0 * boost)
+    return dict(name=f"next4_boosted_{kind}_wave", params=p, prim=finish(p, q), cfl=0.4, steps=None, period=T, var=var, amplitude=A)
 
 
 def reblock(p, prim_blocks, nb):

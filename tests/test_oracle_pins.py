@@ -467,6 +467,55 @@ def test_p9_linear_waves_converge_at_second_order(kind):
     assert slopes[0] > 1.8 and slopes[1] > 1.9, (errs, slopes)
 
 
+# ----------------------------------------------------------------------------- P15
+def _boosted_wave_error(kind, n):
+    w = wl.boosted_linear_wave(n, kind)
+    p = w["params"]
+    r = orc.Run(p, w["prim"])
+    T = w["period"]
+    while r.t < T * (1 - 1e-12):
+        r.step(min(r.dt(0.4), T - r.t))
+    a = wl.from_blocks(p, r.prim)[w["var"]]
+    b = wl.from_blocks(p, w["prim"])[w["var"]]
+    return np.abs(a - b).sum() / n ** 2 / w["amplitude"]     # Eq.61
+
+
+@pytest.mark.parametrize("kind", ["sound", "alfven"])
+def test_p15_boosted_linear_waves_converge_at_second_order(kind):
+    """2-D linear waves on a flat metric with coordinate boosts v_x = v_y = 0.617213 return to the
+    initial condition after one period and converge at "roughly at least the expected second order" in the L1 norm
+    of Eq.61.  Pins the shift-vector plumbing (transport velocity alpha v - beta, signal speeds, CT in 2-D)."""
+    sizes = (32, 64, 128) if kind == "sound" else (32, 64)      # the CPU suite's time budget
+    errs = [_boosted_wave_error(kind, n) for n in sizes]
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(len(sizes) - 1)]
+    print(kind, errs, slopes)
+    assert errs[0] < 0.2, errs                   # the pattern came back where it started
+    assert slopes[0] > 1.7 and slopes[-1] > (1.85 if len(sizes) == 3 else 1.7), (errs, slopes)
+
+
+def test_p15b_boosted_metric_is_a_coordinate_change():
+    """Exact properties of the boosted flat metric: det g = -1, alpha = 1, beta^i = shift^i, gamma_ij = delta_ij; a uniform
+    state (at rest or moving) stays bitwise uniform; with zero shift the run is bitwise the Minkowski one."""
+    p = wl.default_params(metric=wl.MINKOWSKI_BOOSTED, shift=(0.617213, 0.617213, 0.0), nx=12, ny=12, nz=1, ng=2)
+    g = orc.metric(p, [0.3, 0.1, 0.0])
+    assert abs(np.linalg.det(g) + 1.0) < 1e-15
+    sp = orc.split31(g)
+    assert abs(sp["alpha"] - 1.0) < 1e-15 and np.allclose(sp["beta_u"], [0.617213, 0.617213, 0.0], atol=1e-15)
+    assert np.array_equal(sp["gamma_l"], np.eye(3))
+    q = np.zeros((8, 1, 12, 12))
+    q[0], q[1], q[2], q[3], q[4], q[5], q[6], q[7] = 1.3, 0.4, -0.2, 0.1, 2.1, 0.7, -0.3, 0.2
+    o = orc.Run(p, wl.finish(p, q)); c0 = o.cons.copy()
+    o.step(o.dt(0.4))
+    assert np.array_equal(wl.from_blocks(p, o.cons), wl.from_blocks(p, c0))
+    w = wl.turbulence_box(8)
+    p0 = w["params"]; p2 = dict(p0); p2.update(metric=wl.MINKOWSKI_BOOSTED, shift=(0.0, 0.0, 0.0))
+    a = orc.Run(p0, w["prim"]); b = orc.Run(p2, w["prim"])
+    dt = a.dt(0.4)
+    assert b.dt(0.4) == dt
+    a.step(dt); b.step(dt)
+    assert np.array_equal(a.cons, b.cons)
+
+
 # ----------------------------------------------------------------------------- P10
 def _shock_tube(n):
     w = wl.shock_tube(n)
