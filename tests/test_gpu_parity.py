@@ -349,3 +349,28 @@ def test_evolve_host_matches_device_path():
     tt = phx.evolve_host(mesh, hin, 2, 0.4, hp, hc, hm)
     assert tt == t
     assert np.array_equal(hp.numpy(), pb) and np.array_equal(hc.numpy(), cb) and np.array_equal(hm.numpy(), mb)
+
+
+def test_boosted_turbulence_matches_oracle():
+    """A 3-D state with large amplitudes on the boosted flat metric (shift in all three directions): every flux term that
+    carries beta^i is exercised far from the linear regime."""
+    w = wl.turbulence_box(20)
+    p = dict(w["params"]); p.update(metric=wl.MINKOWSKI_BOOSTED, shift=(0.4, -0.3, 0.5))
+    o, g = run_both(p, w["prim"], nsteps=10, cfl=0.4)
+    compare(p, o, g, TOL_100STEP)
+    o1, g1 = run_both(p, w["prim"], nsteps=1, cfl=0.4)
+    compare(p, o1, g1, TOL_1STEP)
+
+
+@pytest.mark.parametrize("kind,recon,n", [("sound", wl.RECON_PLM_MC, 48), ("alfven", wl.RECON_WENO5Z, 40)])
+def test_boosted_linear_waves_match_oracle(kind, recon, n):
+    """2-D linear waves on the boosted flat metric, 1 and 100 steps.  The wave
+    amplitude is 1e-6, so the momentum (1e-6) is the difference of O(1) pressure fluxes: its error is measured against
+    the largest conserved scale (scale_floor = 1), the other variables against their own."""
+    w = wl.boosted_linear_wave(n, kind, recon=recon)
+    p = w["params"]
+    o, g = run_both(p, w["prim"], nsteps=1, cfl=0.4)
+    compare(p, o, g, TOL_1STEP, scale_floor=1.0)
+    o, g = run_both(p, w["prim"], nsteps=100, cfl=0.4)
+    compare(p, o, g, TOL_100STEP, scale_floor=1.0)
+    assert abs(g.dt(0.4) - o.dt(0.4)) <= 1e-13 * o.dt(0.4)
