@@ -67,7 +67,7 @@ __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G
 // ---- x sweep ------------------------------------------------------------------------------------
 // position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
 template <int METRIC, int RECON>
-__global__ void __launch_bounds__(XS_BLOCK, PHX_XS_MINB) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : PHX_XS_MINB)) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
                                                       int nplane, int rowlen, int j0, int k0) {
   // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii)
   constexpr int HW = ReconTraits<RECON>::HW;
