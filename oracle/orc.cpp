@@ -16,8 +16,10 @@
 // P3 corner div B, P4 round trip, P5 algebraic identities against T^{mu nu} of Eq.9, P6
 // Kerr-Schild identities and derivatives, P7 sources against the printed Eq.4 forms, P8 wave
 // speeds against the covariant dispersion relation, P9 linear-wave convergence, P10 shock-tube
-// structure, P11 block invariance, P12 WENO5-Z order.  Parity-unpinned parts: the absolute
-// accuracy of the synthetic configs 3-5 (no printed values exist in the paper for this path).
+// structure, P11 block invariance, P12 WENO5-Z order, P12b/c WENO5-Z-AOAH, P12d MP5, P13 Bondi
+// inflow stationary in Kerr-Schild (a = 0), P14 Sedov-Taylor shock radius, P15 boosted linear waves.
+// Parity-unpinned parts: the absolute accuracy of the synthetic configs 3-5 for spin a != 0 (no
+// printed values exist in the paper for this path, no closed-form solution is used there).
 //
 // Layout of every field: [block][var][k][j][i], i fastest; var order of primitives
 // P=(rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3) (Eq.13) and conserved, stored densitised,

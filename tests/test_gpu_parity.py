@@ -374,3 +374,17 @@ def test_boosted_linear_waves_match_oracle(kind, recon, n):
     o, g = run_both(p, w["prim"], nsteps=100, cfl=0.4)
     compare(p, o, g, TOL_100STEP, scale_floor=1.0)
     assert abs(g.dt(0.4) - o.dt(0.4)) <= 1e-13 * o.dt(0.4)
+
+
+def test_bondi_inflow_matches_oracle_and_stays_stationary():
+    """Pin P13's exact stationary solution (Bondi inflow, Kerr-Schild a = 0) through the CUDA path: parity with the oracle
+    over 12 steps and the same stationarity away from the outflow faces."""
+    from test_oracle_pins import bondi_params, bondi_prims
+    p = bondi_params(24)
+    q = bondi_prims(p)
+    prim = wl.finish(p, q)
+    o, g = run_both(p, prim, nsteps=12, cfl=0.4)
+    compare(p, o, g, TOL_100STEP)
+    q1 = interior(p, g.get()[1])
+    sl = (slice(6, -6),) * 3
+    assert (np.abs(q1[0][sl] - q[0][sl]) / q[0][sl]).max() < 1e-3
