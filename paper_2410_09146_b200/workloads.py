@@ -309,6 +309,8 @@ def sedov_blast(n=128, E=1e-5, r_init=0.1, recon=RECON_PLM_MINMOD):
     q = np.zeros((NV, n, n, n))
     q[0] = 1.0
     q[4] = 1e-7 / (p["gamma_ad"] - 1.0)
+    if not inside.any():
+        raise ValueError("sedov_blast: no cell centre inside r_init at this resolution")
     q[4][inside] += E / (inside.sum() * dV)
     return dict(name="next2_sedov_blast", params=p, prim=finish(p, q), cfl=0.4, steps=20)
 
