@@ -21,6 +21,10 @@
 // Parity-unpinned parts: the absolute accuracy of the synthetic configs 3-5 for spin a != 0 (no
 // printed values exist in the paper for this path, no closed-form solution is used there).
 //
+// P16 passive scalar (Eq.14): constant X stays constant, sum of sqrt(gamma) D X conserved, smooth profile advected at
+// second order, bounds; P17 floor forms of PAPER.md:288 against the closed-form Kerr-Schild radius on the axis, in the
+// equatorial plane and for a = 0.
+//
 // Layout of every field: [block][var][k][j][i], i fastest; var order of primitives
 // P=(rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3) (Eq.13) and conserved, stored densitised,
 // sqrt(gamma)*(D, S_1, S_2, S_3, tau, B^1, B^2, B^3) (Eq.1-2).
@@ -43,6 +47,10 @@ typedef struct {
   double rho_floor, eps_floor, w_max;
   double c2p_tol;  int c2p_maxit;
   double shift[3];   /* metric 2: flat metric in coordinates boosted by x' = x - shift*t */
+  int nscalar;       /* 0 or 1 passive scalar X carried as variable 8 of every field (Eq.14) */
+  double scalar_min, scalar_max;   /* X is kept inside these bounds */
+  int floor_form;    /* 0 rho0; 1 rho0 exp(-alpha x1); 2 rho0 x1^-alpha; 3 rho0 r^-alpha (x1 = r here) */
+  double floor_alpha_rho, floor_alpha_eps;
 } orc_params;
 }
 
@@ -51,7 +59,8 @@ namespace {
 enum { NV = 8, RHO = 0, UX = 1, UY = 2, UZ = 3, UU = 4, BX = 5, BY = 6, BZ = 7 };
 enum { CD = 0, CS1 = 1, CS2 = 2, CS3 = 3, CTAU = 4 };
 enum { M_RHO_FLOOR = 1, M_EPS_FLOOR = 2, M_EPS_CLIPPED = 4, M_W_CEIL = 8, M_NOCONV = 16, M_BAD_INPUT = 32,
-       M_EXCISED = 64 };
+       M_EXCISED = 64, M_SCALAR_CLIPPED = 128 };
+enum { XS = 8, NVMAX = 9 };   // index of the passive scalar (primitive X, conserved sqrt(gamma) D X) when nscalar = 1
 
 double g_last_margin = 1e300;   // smallest relative distance of any c2p decision to its threshold
 
@@ -63,7 +72,9 @@ struct Grid {
   double dx[3];
   long ncell;   // allocated cells per block
   int nblk;
+  int nv;       // variables per field: 8 + nscalar
   explicit Grid(const orc_params& q) : p(q) {
+    nv = NV + (q.nscalar > 0 ? 1 : 0);
     nb[0] = q.nbx; nb[1] = q.nby; nb[2] = q.nbz;
     n[0] = q.nx; n[1] = q.ny; n[2] = q.nz;
     for (int d = 0; d < 3; ++d) {
@@ -77,7 +88,7 @@ struct Grid {
     nblk = nb[0] * nb[1] * nb[2];
   }
   long idx(int b, int v, int k, int j, int i) const {
-    return (((long)b * NV + v) * na[2] + k) * (long)na[1] * na[0] + (long)j * na[0] + i;
+    return (((long)b * nv + v) * na[2] + k) * (long)na[1] * na[0] + (long)j * na[0] + i;
   }
   long cidx(int b, int k, int j, int i) const {   // one-variable arrays (mask)
     return ((long)b * na[2] + k) * (long)na[1] * na[0] + (long)j * na[0] + i;
@@ -392,21 +403,29 @@ void recon_cell(int recon, const double* s, long stride, double& qm, double& qp)
 int stencil_halfwidth(int recon) { return recon == 0 ? 0 : (recon >= 3 ? 2 : 1); }
 
 // ------------------------------------------------------------------------------------------ C5.2
-void riemann_face(const orc_params& p, const Geo& G, int d, const double qL[NV], const double qR[NV], double F[NV]) {
-  double UL[NV], UR[NV], FL[NV], FR[NV], lmL, lpL, lmR, lpR;
+// ns = 1: qL, qR, F carry the passive scalar at index XS.  Eq.14, (X rho u^mu)_{;mu} = 0, in conservation form is
+// d_t (sqrt(gamma) D X) + d_i (sqrt(gamma) D X (alpha v^i - beta^i)) = 0, i.e. for one state U~_X = U~_D X and
+// F~_X = F~_D X; the two states are combined by the same HLL / LLF formula and speeds as every other variable.
+void riemann_face(const orc_params& p, const Geo& G, int d, const double* qL, const double* qR, double* F, int ns = 0) {
+  double UL[NVMAX], UR[NVMAX], FL[NVMAX], FR[NVMAX], lmL, lpL, lmR, lpR;
   cons_at(qL, G, p.gamma_ad, UL); cons_at(qR, G, p.gamma_ad, UR);
   flux_at(qL, G, p.gamma_ad, d, FL); flux_at(qR, G, p.gamma_ad, d, FR);
   speeds_at(qL, G, p.gamma_ad, d, lmL, lpL); speeds_at(qR, G, p.gamma_ad, d, lmR, lpR);
   for (int v = 0; v < NV; ++v) {   // densitise: U~ = sqrt(gamma) U, F~ = alpha sqrt(gamma) F (Eq.1)
     UL[v] *= G.sg; UR[v] *= G.sg; FL[v] *= G.alpha * G.sg; FR[v] *= G.alpha * G.sg;
   }
+  const int nv = NV + (ns ? 1 : 0);
+  if (ns) {
+    UL[XS] = UL[CD] * qL[XS]; UR[XS] = UR[CD] * qR[XS];
+    FL[XS] = FL[CD] * qL[XS]; FR[XS] = FR[CD] * qR[XS];
+  }
   if (p.riemann == 1) {   // HLL
     const double sp = std::fmax(0.0, std::fmax(lpL, lpR));
     const double sm = std::fmin(0.0, std::fmin(lmL, lmR));
-    for (int v = 0; v < NV; ++v) F[v] = (sp * FL[v] - sm * FR[v] + sp * sm * (UR[v] - UL[v])) / (sp - sm);
+    for (int v = 0; v < nv; ++v) F[v] = (sp * FL[v] - sm * FR[v] + sp * sm * (UR[v] - UL[v])) / (sp - sm);
   } else {                // LLF
     const double c = std::fmax(std::fmax(std::fabs(lmL), std::fabs(lpL)), std::fmax(std::fabs(lmR), std::fabs(lpR)));
-    for (int v = 0; v < NV; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * c * (UR[v] - UL[v]);
+    for (int v = 0; v < nv; ++v) F[v] = 0.5 * (FL[v] + FR[v]) - 0.5 * c * (UR[v] - UL[v]);
   }
   F[BX + d] = 0.0;
 }
@@ -502,7 +521,9 @@ void note_margin(double& margin, double value, double threshold) {
 }
 
 // U: densitised conserved at one cell (rewritten when floored), q: primitives out.
-unsigned char c2p_cell(const orc_params& p, const Geo& G, double Ut[NV], double q[NV], double& margin) {
+// rho_flr, eps_flr: the floors at this cell (floors_at).
+unsigned char c2p_cell(const orc_params& p, const Geo& G, double rho_flr, double eps_flr, double Ut[NV], double q[NV],
+                       double& margin) {
   unsigned char mask = 0;
   double U[NV];
   for (int v = 0; v < NV; ++v) U[v] = Ut[v] / G.sg;
@@ -512,7 +533,7 @@ unsigned char c2p_cell(const orc_params& p, const Geo& G, double Ut[NV], double 
   const double Bu[3] = {U[BX], U[BX + 1], U[BX + 2]};
   if (bad) {
     mask |= M_BAD_INPUT;
-    rho = p.rho_floor; eps = p.eps_floor; ut[0] = ut[1] = ut[2] = 0.0;
+    rho = rho_flr; eps = eps_flr; ut[0] = ut[1] = ut[2] = 0.0;
   } else {
     const double D = U[CD];
     C2P c;
@@ -553,15 +574,15 @@ unsigned char c2p_cell(const orc_params& p, const Geo& G, double Ut[NV], double 
     double x, rbar2, qbar; c.aux(mu, x, rbar2, qbar);
     rho = D / W;
     eps = er;
-    note_margin(margin, eps + p.eps_floor, p.eps_floor);   // distance of eps from 0 in units of the floor
+    note_margin(margin, eps + eps_flr, eps_flr);   // distance of eps from 0 in units of the floor
     if (eps < 0.0) { mask |= M_EPS_CLIPPED; eps = 0.0; }
     for (int i = 0; i < 3; ++i) ut[i] = W * mu * x * (ru[i] + mu * c.rb * bu[i]);
   }
-  // floors (constant form)
-  if (!bad) note_margin(margin, rho, p.rho_floor);
-  if (rho < p.rho_floor) { rho = p.rho_floor; mask |= M_RHO_FLOOR; }
-  if (!bad && !(mask & M_EPS_CLIPPED)) note_margin(margin, eps, p.eps_floor);
-  if (eps < p.eps_floor) { eps = p.eps_floor; mask |= M_EPS_FLOOR; }
+  // floors
+  if (!bad) note_margin(margin, rho, rho_flr);
+  if (rho < rho_flr) { rho = rho_flr; mask |= M_RHO_FLOOR; }
+  if (!bad && !(mask & M_EPS_CLIPPED)) note_margin(margin, eps, eps_flr);
+  if (eps < eps_flr) { eps = eps_flr; mask |= M_EPS_FLOOR; }
   double uu = 0.0;
   for (int i = 0; i < 3; ++i) for (int j = 0; j < 3; ++j) uu += G.gl[i][j] * ut[i] * ut[j];
   const double W = std::sqrt(1.0 + uu);
@@ -581,24 +602,66 @@ unsigned char c2p_cell(const orc_params& p, const Geo& G, double Ut[NV], double 
   return mask;
 }
 
+// Floor forms of PAPER.md:288: rho_flr = rho0, rho0 exp(-alpha x^1), rho0 (x^1)^-alpha, rho0 r^-alpha, "the specific
+// internal energy is set similarly" with its own exponent.  The coordinates here are Cartesian, so the
+// "radial coordinate x^1" is read as r (reading C8b): the Kerr-Schild radius for metric 1, the Euclidean
+// distance from the origin for the flat metrics; forms 2 and 3 therefore coincide.
+void floors_at(const orc_params& p, const double x[3], double& rho_flr, double& eps_flr) {
+  rho_flr = p.rho_floor; eps_flr = p.eps_floor;
+  if (p.floor_form == 0) return;
+  double r;
+  if (p.metric == 1) { double H, l[4]; ks_scalars(p, x, r, H, l); }
+  else r = std::sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+  if (p.floor_form == 1) {
+    rho_flr = p.rho_floor * std::exp(-p.floor_alpha_rho * r);
+    eps_flr = p.eps_floor * std::exp(-p.floor_alpha_eps * r);
+  } else {
+    rho_flr = p.rho_floor * std::pow(r, -p.floor_alpha_rho);
+    eps_flr = p.eps_floor * std::pow(r, -p.floor_alpha_eps);
+  }
+}
+
+// Passive scalar of one cell after con2prim (Eq.14; bounds PAPER.md:290 "we simply require that it stay within the
+// bounds").  Dt_in: sqrt(gamma) D the update produced (before any floor), Dt_out: after the floors.
+// X = (sqrt(gamma) D X) / (sqrt(gamma) D), clipped to [scalar_min, scalar_max] (bit 128; a non-finite X or a bad cell goes
+// to scalar_min); where a floor, the ceiling or the clip acted, the conserved scalar is recomputed as Dt_out * X.
+void scalar_recover(const orc_params& p, double Dt_in, double Dt_out, unsigned char& mask, double& UX, double& X,
+                    double& margin) {
+  if (mask & M_BAD_INPUT) {
+    X = p.scalar_min;
+    mask |= M_SCALAR_CLIPPED;
+  } else {
+    X = UX / Dt_in;
+    const double range = p.scalar_max - p.scalar_min;
+    if (std::isfinite(X)) {
+      const double m = std::fmin(std::fabs(X - p.scalar_min), std::fabs(X - p.scalar_max)) / range;
+      if (m < margin) margin = m;
+    }
+    if (!(X >= p.scalar_min)) { X = p.scalar_min; mask |= M_SCALAR_CLIPPED; }
+    else if (X > p.scalar_max) { X = p.scalar_max; mask |= M_SCALAR_CLIPPED; }
+  }
+  if (mask & (M_RHO_FLOOR | M_EPS_FLOOR | M_W_CEIL | M_BAD_INPUT | M_SCALAR_CLIPPED)) UX = Dt_out * X;
+}
+
 // ------------------------------------------------------------------------------------------ C9
 // Ghost fill through the global array: gather block interiors, fill x then y then z (periodic wrap
 // or zero-gradient copy, including already-filled ghosts), scatter every block's ghost frame.
 void fill_ghosts(const Grid& G, double* prim) {
   const int* g = G.g;
   const long NA[3] = {G.N[0] + 2 * g[0], G.N[1] + 2 * g[1], G.N[2] + 2 * g[2]};
-  std::vector<double> glob((size_t)NV * NA[0] * NA[1] * NA[2]);
+  const int NVg = G.nv;
+  std::vector<double> glob((size_t)NVg * NA[0] * NA[1] * NA[2]);
   auto gid = [&](int v, long k, long j, long i) { return ((v * NA[2] + k) * NA[1] + j) * NA[0] + i; };
   for (int b = 0; b < G.nblk; ++b) {
     int c[3]; G.bcoord(b, c);
-    for (int v = 0; v < NV; ++v)
+    for (int v = 0; v < NVg; ++v)
       for (int k = 0; k < G.n[2]; ++k) for (int j = 0; j < G.n[1]; ++j) for (int i = 0; i < G.n[0]; ++i)
         glob[gid(v, c[2] * G.n[2] + k + g[2], c[1] * G.n[1] + j + g[1], c[0] * G.n[0] + i + g[0])] =
             prim[G.idx(b, v, k + g[2], j + g[1], i + g[0])];
   }
   for (int d = 0; d < 3; ++d) {
     if (g[d] == 0) continue;
-    for (int v = 0; v < NV; ++v)
+    for (int v = 0; v < NVg; ++v)
       for (long k = 0; k < NA[2]; ++k) for (long j = 0; j < NA[1]; ++j) for (long i = 0; i < NA[0]; ++i) {
         long c[3] = {i, j, k};
         // only cells whose later-dimension indices are interior or whose earlier dims are anything
@@ -616,7 +679,7 @@ void fill_ghosts(const Grid& G, double* prim) {
   }
   for (int b = 0; b < G.nblk; ++b) {
     int c[3]; G.bcoord(b, c);
-    for (int v = 0; v < NV; ++v)
+    for (int v = 0; v < NVg; ++v)
       for (int k = 0; k < G.na[2]; ++k) for (int j = 0; j < G.na[1]; ++j) for (int i = 0; i < G.na[0]; ++i) {
         const bool interior = k >= g[2] && k < g[2] + G.n[2] && j >= g[1] && j < g[1] + G.n[1] && i >= g[0] && i < g[0] + G.n[0];
         if (interior) continue;
@@ -644,11 +707,12 @@ void block_fluxes(const Grid& G, int b, const double* prim, std::vector<double> 
   const double* P = prim + G.idx(b, 0, 0, 0, 0);
   auto cid = [&](int k, int j, int i) { return (long)k * str[2] + (long)j * str[1] + i; };
   const bool par = (long)n[1] * n[2] > 1;
+  const int nv = G.nv, ns = G.nv - NV;
   for (int d = 0; d < 3; ++d) {
-    F[d].assign((size_t)NV * vstr, 0.0);
+    F[d].assign((size_t)nv * vstr, 0.0);
     if (!G.act[d]) continue;
-    // 1. reconstruct every cell that borders a needed face
-    std::vector<double> qm((size_t)NV * vstr, 0.0), qp((size_t)NV * vstr, 0.0);
+    // 1. reconstruct every cell that borders a needed face (the passive scalar like any other primitive)
+    std::vector<double> qm((size_t)nv * vstr, 0.0), qp((size_t)nv * vstr, 0.0);
     int lo[3], hi[3];   // cell ranges (inclusive)
     for (int e = 0; e < 3; ++e) {
       lo[e] = G.act[e] ? g[e] - 1 : 0;
@@ -659,15 +723,18 @@ void block_fluxes(const Grid& G, int b, const double* prim, std::vector<double> 
       for (int j = lo[1]; j <= hi[1]; ++j)
         for (int i = lo[0]; i <= hi[0]; ++i) {
           const long c = cid(k, j, i);
-          double m[NV], pl[NV];
-          for (int v = 0; v < NV; ++v) recon_cell(p.recon, P + v * vstr + c, str[d], m[v], pl[v]);
+          double m[NVMAX], pl[NVMAX];
+          for (int v = 0; v < nv; ++v) recon_cell(p.recon, P + v * vstr + c, str[d], m[v], pl[v]);
           if (p.recon >= 3) {
-            // positivity fallback: piecewise constant in this direction for all variables
-            if (m[RHO] <= p.rho_floor || pl[RHO] <= p.rho_floor || m[UU] <= p.rho_floor * p.eps_floor ||
-                pl[UU] <= p.rho_floor * p.eps_floor)
-              for (int v = 0; v < NV; ++v) m[v] = pl[v] = P[v * vstr + c];
+            // positivity fallback: piecewise constant in this direction for all variables; the thresholds are the
+            // floors at the centre of the cell
+            const double xc[3] = {G.xc(0, b, i), G.xc(1, b, j), G.xc(2, b, k)};
+            double rfl, efl;
+            floors_at(p, xc, rfl, efl);
+            if (m[RHO] <= rfl || pl[RHO] <= rfl || m[UU] <= rfl * efl || pl[UU] <= rfl * efl)
+              for (int v = 0; v < nv; ++v) m[v] = pl[v] = P[v * vstr + c];
           }
-          for (int v = 0; v < NV; ++v) { qm[v * vstr + c] = m[v]; qp[v * vstr + c] = pl[v]; }
+          for (int v = 0; v < nv; ++v) { qm[v * vstr + c] = m[v]; qp[v * vstr + c] = pl[v]; }
         }
     // 2. Riemann problem at every face (i-1/2) along d, i in [g, g+n]
     int flo[3], fhi[3];
@@ -682,10 +749,10 @@ void block_fluxes(const Grid& G, int b, const double* prim, std::vector<double> 
           const int il[3] = {i, j, k};
           x[d] = G.xf(d, b, il[d]);
           const Geo geo = geo_at(p, x);
-          double qL[NV], qR[NV], Ff[NV];
-          for (int v = 0; v < NV; ++v) { qL[v] = qp[v * vstr + c - str[d]]; qR[v] = qm[v * vstr + c]; }
-          riemann_face(p, geo, d, qL, qR, Ff);
-          for (int v = 0; v < NV; ++v) F[d][v * vstr + c] = Ff[v];
+          double qL[NVMAX], qR[NVMAX], Ff[NVMAX];
+          for (int v = 0; v < nv; ++v) { qL[v] = qp[v * vstr + c - str[d]]; qR[v] = qm[v * vstr + c]; }
+          riemann_face(p, geo, d, qL, qR, Ff, ns);
+          for (int v = 0; v < nv; ++v) F[d][v * vstr + c] = Ff[v];
         }
   }
   // 3. flux-CT (Toth 2000, cell-centred field)
@@ -755,11 +822,12 @@ void rk_stage(const Grid& G, double g0, double g1, double bdt, const double* con
           const long c = (long)k * str[2] + (long)j * str[1] + i;
           if (excised(G, b, k, j, i)) { mask[G.cidx(b, k, j, i)] = M_EXCISED; continue; }
           const double x[3] = {G.xc(0, b, i), G.xc(1, b, j), G.xc(2, b, k)};
-          double R[NV];
-          for (int v = 0; v < NV; ++v) R[v] = 0.0;
+          const int nv = G.nv;
+          double R[NVMAX];
+          for (int v = 0; v < nv; ++v) R[v] = 0.0;
           for (int d = 0; d < 3; ++d) {
             if (!G.act[d]) continue;
-            for (int v = 0; v < NV; ++v) R[v] -= (F[d][v * vstr + c + str[d]] - F[d][v * vstr + c]) / G.dx[d];
+            for (int v = 0; v < nv; ++v) R[v] -= (F[d][v * vstr + c + str[d]] - F[d][v * vstr + c]) / G.dx[d];
           }
           if (p.metric != 0) {
             double g4[4][4], dg[3][4][4], q[NV], S[NV];
@@ -769,16 +837,20 @@ void rk_stage(const Grid& G, double g0, double g1, double bdt, const double* con
             source_at(q, g4, dg, p.gamma_ad, S);
             for (int v = 0; v < NV; ++v) R[v] += S[v];
           }
-          double U[NV], q[NV];
-          for (int v = 0; v < NV; ++v) {
+          double U[NVMAX], q[NVMAX];
+          for (int v = 0; v < nv; ++v) {   // the scalar has no source (S = 0 in Eq.14: no neutrino exchange on this path)
             const long id = G.idx(b, v, k, j, i);
             U[v] = g0 * cons0[id] + g1 * cons[id] + bdt * R[v];
           }
           const Geo geo = geo_at(p, x);
-          const unsigned char m = c2p_cell(p, geo, U, q, marg);   // 6. con2prim + floors
+          double rfl, efl;
+          floors_at(p, x, rfl, efl);
+          const double Dt_in = U[CD];
+          unsigned char m = c2p_cell(p, geo, rfl, efl, U, q, marg);   // 6. con2prim + floors
+          if (nv > NV) scalar_recover(p, Dt_in, U[CD], m, U[XS], q[XS], marg);
           // this block's fluxes are complete and every block reads ghosts from its own storage,
           // so the interior primitives may be overwritten now
-          for (int v = 0; v < NV; ++v) { cons[G.idx(b, v, k, j, i)] = U[v]; prim[G.idx(b, v, k, j, i)] = q[v]; }
+          for (int v = 0; v < nv; ++v) { cons[G.idx(b, v, k, j, i)] = U[v]; prim[G.idx(b, v, k, j, i)] = q[v]; }
           mask[G.cidx(b, k, j, i)] = m;
         }
     if (marg < g_last_margin) g_last_margin = marg;
@@ -791,7 +863,7 @@ void rk_stage(const Grid& G, double g0, double g1, double bdt, const double* con
 // ============================================================================================
 extern "C" {
 
-size_t orc_field_elems(const orc_params* p) { Grid G(*p); return (size_t)G.nblk * NV * G.ncell; }
+size_t orc_field_elems(const orc_params* p) { Grid G(*p); return (size_t)G.nblk * G.nv * G.ncell; }
 double orc_last_c2p_margin(void) { return g_last_margin; }
 void orc_reset_c2p_margin(void) { g_last_margin = 1e300; }
 
@@ -807,6 +879,7 @@ int orc_prim_to_cons(const orc_params* p, const double* prim, double* cons) {
       for (int v = 0; v < NV; ++v) q[v] = prim[G.idx(b, v, k, j, i)];
       cons_at(q, geo, p->gamma_ad, U);
       for (int v = 0; v < NV; ++v) cons[G.idx(b, v, k, j, i)] = geo.sg * U[v];
+      if (G.nv > NV) cons[G.idx(b, XS, k, j, i)] = geo.sg * U[CD] * prim[G.idx(b, XS, k, j, i)];   // sqrt(gamma) D X (Eq.14)
     }
   return 0;
 }
@@ -823,10 +896,15 @@ int orc_cons_to_prim(const orc_params* p, double* cons, double* prim, unsigned c
           if (excised(G, b, k, j, i)) { mask[G.cidx(b, k, j, i)] = M_EXCISED; continue; }
           const double x[3] = {G.xc(0, b, i), G.xc(1, b, j), G.xc(2, b, k)};
           const Geo geo = geo_at(*p, x);
-          double U[NV], q[NV];
-          for (int v = 0; v < NV; ++v) U[v] = cons[G.idx(b, v, k, j, i)];
-          mask[G.cidx(b, k, j, i)] = c2p_cell(*p, geo, U, q, marg);
-          for (int v = 0; v < NV; ++v) { cons[G.idx(b, v, k, j, i)] = U[v]; prim[G.idx(b, v, k, j, i)] = q[v]; }
+          double U[NVMAX], q[NVMAX];
+          for (int v = 0; v < G.nv; ++v) U[v] = cons[G.idx(b, v, k, j, i)];
+          double rfl, efl;
+          floors_at(*p, x, rfl, efl);
+          const double Dt_in = U[CD];
+          unsigned char m = c2p_cell(*p, geo, rfl, efl, U, q, marg);
+          if (G.nv > NV) scalar_recover(*p, Dt_in, U[CD], m, U[XS], q[XS], marg);
+          mask[G.cidx(b, k, j, i)] = m;
+          for (int v = 0; v < G.nv; ++v) { cons[G.idx(b, v, k, j, i)] = U[v]; prim[G.idx(b, v, k, j, i)] = q[v]; }
         }
   if (marg < g_last_margin) g_last_margin = marg;
   fill_ghosts(G, prim);
@@ -876,7 +954,7 @@ int orc_stage_fluxes(const orc_params* p, const double* prim, double* F1, double
   for (int b = 0; b < G.nblk; ++b) {
     std::vector<double> F[3];
     block_fluxes(G, b, prim, F);
-    for (int d = 0; d < 3; ++d) std::memcpy(out[d] + G.idx(b, 0, 0, 0, 0), F[d].data(), sizeof(double) * NV * G.ncell);
+    for (int d = 0; d < 3; ++d) std::memcpy(out[d] + G.idx(b, 0, 0, 0, 0), F[d].data(), sizeof(double) * G.nv * G.ncell);
   }
   return 0;
 }
@@ -921,13 +999,20 @@ void orc_point_stress_energy(const double* g16, double gam, const double* q, dou
 int orc_point_c2p(const orc_params* p, const double* g16, double* U, double* q) {
   double g[4][4]; std::memcpy(g, g16, sizeof g);
   double marg = 1e300;
-  const int m = c2p_cell(*p, split31(g), U, q, marg);
+  const int m = c2p_cell(*p, split31(g), p->rho_floor, p->eps_floor, U, q, marg);   // constant-form floors
   if (marg < g_last_margin) g_last_margin = marg;
   return m;
 }
 void orc_point_riemann(const orc_params* p, const double* g16, int d, const double* qL, const double* qR, double* F) {
   double g[4][4]; std::memcpy(g, g16, sizeof g);
   riemann_face(*p, split31(g), d, qL, qR, F);
+}
+// floors at a point (PAPER.md:288 forms)
+void orc_point_floors(const orc_params* p, const double* x, double* rho_flr, double* eps_flr) { floors_at(*p, x, *rho_flr, *eps_flr); }
+// Riemann flux of the 8 variables plus the passive scalar (qL, qR, F: 9 entries)
+void orc_point_riemann_scalar(const orc_params* p, const double* g16, int d, const double* qL, const double* qR, double* F) {
+  double g[4][4]; std::memcpy(g, g16, sizeof g);
+  riemann_face(*p, split31(g), d, qL, qR, F, 1);
 }
 // reconstruct a line f[0..n-1]: qm[i], qp[i] for cells with a full stencil (others untouched)
 void orc_recon_line(int recon, int n, const double* f, double* qm, double* qp) {

@@ -26,16 +26,19 @@ class Params(C.Structure):
         ("gamma_ad", C.c_double), ("recon", C.c_int), ("riemann", C.c_int), ("use_ct", C.c_int),
         ("rho_floor", C.c_double), ("eps_floor", C.c_double), ("w_max", C.c_double),
         ("c2p_tol", C.c_double), ("c2p_maxit", C.c_int), ("shift", C.c_double * 3),
+        ("nscalar", C.c_int), ("scalar_min", C.c_double), ("scalar_max", C.c_double),
+        ("floor_form", C.c_int), ("floor_alpha_rho", C.c_double), ("floor_alpha_eps", C.c_double),
     ]
+
+# parameters added after the first version of the ABI: optional in the dictionaries, with the values that switch them off
+_OPTIONAL = dict(shift=(0.0, 0.0, 0.0), nscalar=0, scalar_min=0.0, scalar_max=1.0, floor_form=0,
+                 floor_alpha_rho=2.0, floor_alpha_eps=1.0)
 
 
 def make_params(p: dict) -> Params:
     q = Params()
     for name, _ in Params._fields_:
-        if name == "shift":
-            v = p.get("shift", (0.0, 0.0, 0.0))
-        else:
-            v = p[name]
+        v = p.get(name, _OPTIONAL[name]) if name in _OPTIONAL else p[name]
         if name in ("xmin", "xmax", "shift"):
             setattr(q, name, (C.c_double * 3)(*v))
         elif name == "bc":
@@ -84,6 +87,8 @@ def lib():
         L.orc_point_c2p.restype = C.c_int
         L.orc_point_riemann.argtypes = [pp, dp, C.c_int, dp, dp, dp]
         L.orc_recon_line.argtypes = [C.c_int, C.c_int, dp, dp, dp]
+        L.orc_point_floors.argtypes = [pp, dp, dp, dp]
+        L.orc_point_riemann_scalar.argtypes = [pp, dp, C.c_int, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -233,6 +238,21 @@ def point_riemann(p, g4, d, qL, qR):
     F = np.zeros(8); g4 = np.ascontiguousarray(g4)
     qL = np.ascontiguousarray(qL, dtype=np.float64); qR = np.ascontiguousarray(qR, dtype=np.float64)
     lib().orc_point_riemann(C.byref(make_params(p)), _d(g4), d, _d(qL), _d(qR), _d(F))
+    return F
+
+
+def point_floors(p, x):
+    """(rho_flr, eps_flr) at the point x (PAPER.md:288 forms)."""
+    x = np.asarray(x, dtype=np.float64); r, e = C.c_double(), C.c_double()
+    lib().orc_point_floors(C.byref(make_params(p)), _d(x), C.byref(r), C.byref(e))
+    return r.value, e.value
+
+
+def point_riemann_scalar(p, g4, d, qL, qR):
+    """Riemann flux of the 8 variables and the passive scalar (9 entries in, 9 out)."""
+    F = np.zeros(9); g4 = np.ascontiguousarray(g4)
+    qL = np.ascontiguousarray(qL, dtype=np.float64); qR = np.ascontiguousarray(qR, dtype=np.float64)
+    lib().orc_point_riemann_scalar(C.byref(make_params(p)), _d(g4), d, _d(qL), _d(qR), _d(F))
     return F
 
 

@@ -9,7 +9,8 @@ region and to turn the divergence-free densitised field into the primitive B) ar
 the recipe stated in DESIGN.md section 4.
 
 Layout of every field: [block][var][k][j][i], i fastest, fp64, var order
-(rho, u~1, u~2, u~3, u=rho*eps, B1, B2, B3)  (PAPER.md:111, Eq.13).
+(rho, u~1, u~2, u~3, u=rho*eps, B1, B2, B3)  (Eq.13), plus the passive scalar X
+(Eq.14) as variable 8 when params["nscalar"] = 1.
 Block id = (bz*nby + by)*nbx + bx.  A dimension with one zone in total is inactive and has
 no ghost zones.
 """
@@ -50,7 +51,7 @@ def ghosts(p):
 def alloc_shape(p):
     gx, gy, gz = ghosts(p)
     nb = p["nbx"] * p["nby"] * p["nbz"]
-    return (nb, NV, p["nz"] + 2 * gz, p["ny"] + 2 * gy, p["nx"] + 2 * gx)
+    return (nb, NV + (1 if p.get("nscalar", 0) else 0), p["nz"] + 2 * gz, p["ny"] + 2 * gy, p["nx"] + 2 * gx)
 
 
 def n_zones(p):
@@ -352,6 +353,31 @@ def boosted_linear_wave(n=64, kind="sound", boost=0.617213, A=1e-6, recon=RECON_
         raise ValueError(kind)
     T = 1.0 / (np.sqrt(2.0) * lam + 2.0 * boost)
     return dict(name=f"next4_boosted_{kind}_wave", params=p, prim=finish(p, q), cfl=0.4, steps=None, period=T, var=var, amplitude=A)
+
+
+def with_scalar(w, X, scalar_min=0.0, scalar_max=1.0):
+    """Workload `w` with a passive scalar (Eq.14; the paper's use is the electron fraction Y_e)
+    appended as variable 8.  X: global interior array [Nz, Ny, Nx] of the advected quantity."""
+    p0 = w["params"]
+    q = np.concatenate([from_blocks(p0, w["prim"]), np.asarray(X, dtype=np.float64)[None]], axis=0)
+    p = dict(p0, nscalar=1, scalar_min=float(scalar_min), scalar_max=float(scalar_max))
+    return dict(w, name=w["name"] + "_scalar", params=p, prim=finish(p, q))
+
+
+def smooth_scalar(p, seed, lo=0.1, hi=0.5):
+    """A seeded smooth field in [lo, hi] on the global interior grid: a few low random Fourier modes (Y_e-like values)."""
+    rng = np.random.default_rng(seed)
+    x, y, z = cell_centres(p)
+    L = [p["xmax"][d] - p["xmin"][d] for d in range(3)]
+    X = np.zeros((len(z), len(y), len(x)))
+    for _ in range(4):
+        k = rng.integers(0, 3, size=3)
+        ph = rng.uniform(0.0, 2.0 * np.pi, size=3)
+        X += (np.cos(2 * np.pi * k[0] * (x - p["xmin"][0]) / L[0] + ph[0])[None, None, :]
+              * np.cos(2 * np.pi * k[1] * (y - p["xmin"][1]) / L[1] + ph[1])[None, :, None]
+              * np.cos(2 * np.pi * k[2] * (z - p["xmin"][2]) / L[2] + ph[2])[:, None, None])
+    X = (X - X.min()) / max(X.max() - X.min(), 1e-300)
+    return lo + (hi - lo) * X
 
 
 def reblock(p, prim_blocks, nb):
