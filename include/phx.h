@@ -7,9 +7,12 @@
  * never throws or aborts; phx_last_error() returns a thread-local message for the last failure.
  * Numerical trouble is never an error code: it is reported per cell in the mask.
  *
- * Field layout (all fp64): [block][var][k][j][i], i fastest, 8 variables, ghosts included.
- *   primitives  P  = (rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3)            PAPER.md:111-113 (Eq.13)
- *   conserved   U~ = sqrt(gamma) * (D, S_1, S_2, S_3, tau, B^1, B^2, B^3)           PAPER.md:59-63 (Eq.1-2)
+ * Field layout (all fp64): [block][var][k][j][i], i fastest, 8 + nscalar variables, ghosts included.
+ *   primitives  P  = (rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3 [, X])      PAPER.md:111-113 (Eq.13)
+ *   conserved   U~ = sqrt(gamma) * (D, S_1, S_2, S_3, tau, B^1, B^2, B^3 [, D X])   PAPER.md:59-63 (Eq.1-2)
+ * X is the passive scalar of Eq.14 (the paper's use is the electron fraction), present as
+ * variable 8 of every field when params.nscalar = 1: (X rho u^mu)_{;mu} = 0, i.e. sqrt(gamma) D X is advected with
+ * the mass flux, F~_X = F~_D X per state, combined by the same LLF / HLL formula as every other variable.
  * Block id = (bz*nby + by)*nbx + bx.  A dimension with one zone in the whole domain is inactive:
  * it has no ghost zones and no sweep.  Ghosts of U~ are never read or written.
  * Mask layout: [block][k][j][i] (uint8, same cell indexing as one variable).
@@ -36,8 +39,14 @@ enum { PHX_BC_PERIODIC = 0, PHX_BC_OUTFLOW = 1 };
 /* con2prim / floor mask bits */
 enum {
   PHX_M_RHO_FLOOR = 1, PHX_M_EPS_FLOOR = 2, PHX_M_EPS_CLIPPED = 4, PHX_M_W_CEIL = 8,
-  PHX_M_NOCONV = 16, PHX_M_BAD_INPUT = 32, PHX_M_EXCISED = 64
+  PHX_M_NOCONV = 16, PHX_M_BAD_INPUT = 32, PHX_M_EXCISED = 64,
+  PHX_M_SCALAR_CLIPPED = 128   /* the passive scalar left [scalar_min, scalar_max] and was put back */
 };
+/* floor forms of PAPER.md:288: rho_flr = rho0 | rho0 exp(-alpha x^1) | rho0 (x^1)^-alpha | rho0 r^-alpha, and "the specific
+ * internal energy is set similarly".  The coordinates of this library are Cartesian, so the radial coordinate
+ * x^1 is read as r: the Kerr-Schild radius for PHX_KERR_SCHILD, the Euclidean distance from the origin for the flat
+ * metrics (forms 2 and 3 coincide).  rho0 = rho_floor, eps0 = eps_floor. */
+enum { PHX_FLOOR_CONST = 0, PHX_FLOOR_EXP_X1 = 1, PHX_FLOOR_POW_X1 = 2, PHX_FLOOR_POW_R = 3 };
 
 typedef struct {
   int metric;
@@ -53,18 +62,23 @@ typedef struct {
   double c2p_tol;                     /* relative tolerance on the con2prim root mu */
   int c2p_maxit;
   double shift[3];                    /* PHX_MINKOWSKI_BOOSTED only: the constant shift vector, |shift| < 1 */
+  int nscalar;                        /* 0 or 1 passive scalar (Eq.14) carried as variable 8 of every field */
+  double scalar_min, scalar_max;      /* after recovery X = U~_X / U~_D is clipped to these bounds (mask bit 128); where a
+                                         floor, the ceiling or the clip acted U~_X is rewritten as U~_D X */
+  int floor_form;                     /* PHX_FLOOR_*; 0 keeps rho_floor and eps_floor constant */
+  double floor_alpha_rho, floor_alpha_eps; /* exponents alpha of the density and specific-energy floors (paper: 2.0) */
 } phx_params;
 
-/* Build a mesh object: validates the parameters, allocates flux scratch (3 x one 8-variable field),
+/* Build a mesh object: validates the parameters, allocates flux scratch (3 x one field),
  * the excision flag array and reduction scratch, and runs the geometry-flag kernel on `stream`.
  * Errors: PHX_EINVAL (bad sizes, ng too small for recon, inactive dimension split over blocks),
  * PHX_ENOMEM, PHX_ECUDA.  The mesh is freed with phx_free_mesh. */
 int phx_init_mesh(const phx_params* params, void* stream, phx_mesh** out);
 int phx_free_mesh(phx_mesh* mesh);
 
-/* Number of doubles in one 8-variable field: nblocks*8*(nz+2gz)*(ny+2gy)*(nx+2gx). */
+/* Number of doubles in one field: nblocks*(8+nscalar)*(nz+2gz)*(ny+2gy)*(nx+2gx). */
 size_t phx_field_elems(const phx_mesh* mesh);
-/* Number of bytes in one mask: phx_field_elems/8. */
+/* Number of bytes in one mask: nblocks*(nz+2gz)*(ny+2gy)*(nx+2gx). */
 size_t phx_mask_elems(const phx_mesh* mesh);
 
 /* U~ = sqrt(gamma) U(P) (Eq.2) at every allocated cell (ghosts included). */

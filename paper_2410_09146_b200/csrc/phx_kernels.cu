@@ -44,38 +44,48 @@ constexpr int XS_BLOCK = PHX_XS_BLOCK;   // threads per block of the x sweep (XS
 constexpr int MS_BLOCK = PHX_MS_BLOCK;   // threads per block of the marching sweeps
 constexpr int UP_BLOCK = PHX_UP_BLOCK;
 
-template <int RECON>
-__device__ __forceinline__ void positivity_fallback(const MeshDev& m, const double* centre, double* qm, double* qp) {
+// (x, y, z): centre of the cell, used only when the floors depend on the position (floor_form != 0)
+template <int METRIC, int RECON, int NS>
+__device__ __forceinline__ void positivity_fallback(const MeshDev& m, double x, double y, double z, const double* centre, double* qm,
+                                                    double* qp) {
   if constexpr (RECON >= 3) {
-    const double ufl = m.rho_floor * m.eps_floor;
-    if (qm[RHO] <= m.rho_floor || qp[RHO] <= m.rho_floor || qm[UU] <= ufl || qp[UU] <= ufl) {
+    double rfl, efl;
+    floors_at<METRIC>(m, x, y, z, rfl, efl);
+    const double ufl = rfl * efl;
+    if (qm[RHO] <= rfl || qp[RHO] <= rfl || qm[UU] <= ufl || qp[UU] <= ufl) {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) { qm[v] = centre[v]; qp[v] = centre[v]; }
+      for (int v = 0; v < NV + NS; ++v) { qm[v] = centre[v]; qp[v] = centre[v]; }
     }
   }
 }
 
-template <int METRIC, int D>
+// NS = 1: qL, qR, F carry the passive scalar at index XS; per state U~_X = U~_D X and F~_X = F~_D X (Eq.14)
+template <int METRIC, int D, int NS>
 __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G, const double* qL, const double* qR, double* F) {
-  double UL[NV], UR[NV], FL[NV], FR[NV], lmL, lpL, lmR, lpR;
+  double UL[NV + NS], UR[NV + NS], FL[NV + NS], FR[NV + NS], lmL, lpL, lmR, lpR;
   state_flux<METRIC, D>(qL, G, m.gam, UL, FL, lmL, lpL);
   state_flux<METRIC, D>(qR, G, m.gam, UR, FR, lmR, lpR);
-  riemann_combine(m.riemann, UL, UR, FL, FR, lmL, lpL, lmR, lpR, F);
+  if constexpr (NS == 1) {
+    UL[XS] = UL[CD] * qL[XS]; UR[XS] = UR[CD] * qR[XS];
+    FL[XS] = FL[CD] * qL[XS]; FR[XS] = FR[CD] * qR[XS];
+  }
+  riemann_combine<NS>(m.riemann, UL, UR, FL, FR, lmL, lpL, lmR, lpR, F);
   F[BX + D] = 0.0;
 }
 
 // ---- x sweep ------------------------------------------------------------------------------------
 // position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
-template <int METRIC, int RECON>
+template <int METRIC, int RECON, int NS>
 __global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : PHX_XS_MINB)) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
                                                       int nplane, int rowlen, int j0, int k0) {
   // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii)
   constexpr int HW = ReconTraits<RECON>::HW;
-  __shared__ double sh[NV][XS_BLOCK];
+  __shared__ double sh[NV + NS][XS_BLOCK];
   const int t = threadIdx.x;
   const int p = blockIdx.x * (XS_BLOCK - 1) + t;
   const bool valid = p < nplane;
-  double qm[NV], qp[NV];
+  constexpr int NQ = NV + NS;
+  double qm[NQ], qp[NQ];
   long long base = 0;
   int ii = 0, i = 0, j = 0, k = 0;
   const int b = blockIdx.z;
@@ -84,33 +94,41 @@ __global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : PHX_XS_MINB)) k_sw
     const int jj = p / rowlen;
     ii = p - jj * rowlen;
     i = m.g[0] - 1 + ii; j = j0 + jj; k = k0 + kk;
-    base = (long long)b * NV * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
-    double centre[NV];
+    base = (long long)b * m.nvar * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
+    double centre[NQ];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NQ; ++v) {
       double f[2 * HW + 1];
 #pragma unroll
       for (int s = 0; s <= 2 * HW; ++s) f[s] = prim[base + v * m.ncell + (s - HW)];
       centre[v] = f[HW];
       recon1<RECON>(f, qm[v], qp[v]);
     }
-    positivity_fallback<RECON>(m, centre, qm, qp);
+    {
+      int cbc[3];
+      double xc = 0.0, yc = 0.0, zc = 0.0;
+      if (RECON >= 3 && m.floor_form != 0) {
+        block_coords(m, b, cbc);
+        xc = xcen(m, 0, cbc[0], i); yc = xcen(m, 1, cbc[1], j); zc = xcen(m, 2, cbc[2], k);
+      }
+      positivity_fallback<METRIC, RECON, NS>(m, xc, yc, zc, centre, qm, qp);
+    }
 #pragma unroll
-    for (int v = 0; v < NV; ++v) sh[v][t] = qp[v];
+    for (int v = 0; v < NQ; ++v) sh[v][t] = qp[v];
   }
   __syncthreads();
   if (!valid || t == 0 || ii == 0) return;
-  double qL[NV];
+  double qL[NQ];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) qL[v] = sh[v][t - 1];
+  for (int v = 0; v < NQ; ++v) qL[v] = sh[v][t - 1];
   int cb[3];
   block_coords(m, b, cb);
   Geo<METRIC> G;
   G.at(m, xface(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
-  double F[NV];
-  face_flux<METRIC, 0>(m, G, qL, qm, F);
+  double F[NQ];
+  face_flux<METRIC, 0, NS>(m, G, qL, qm, F);
 #pragma unroll
-  for (int v = 0; v < NV; ++v) flux[base + v * m.ncell] = F[v];
+  for (int v = 0; v < NQ; ++v) flux[base + v * m.ncell] = F[v];
 }
 
 // ---- y / z sweep ---------------------------------------------------------------------------------
@@ -127,13 +145,14 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-template <int METRIC, int RECON, int D>
+template <int METRIC, int RECON, int D, int NS>
 __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
                                                                        int ntr, int n0, int lo0, int lo1, int L) {
   constexpr int HW = ReconTraits<RECON>::HW;
   constexpr int NW = 2 * HW + 1;   // stencil rows
   constexpr int NR = NW + 1;       // ring: the stencil plus one row in flight
-  __shared__ double win[NR][NV][MS_BLOCK];
+  constexpr int NQ = NV + NS;
+  __shared__ double win[NR][NQ][MS_BLOCK];
   const int tid = threadIdx.x;
   const int p = blockIdx.x * MS_BLOCK + tid;
   if (p >= ntr) return;
@@ -147,7 +166,7 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
   const int f0 = m.g[D] + seg * L;
   const int f1 = min(f0 + L - 1, m.g[D] + m.n[D]);
   if (f0 > f1) return;
-  const long long col = (long long)b * NV * m.ncell + (long long)o * so + i;
+  const long long col = (long long)b * m.nvar * m.ncell + (long long)o * so + i;
   int cb[3];
   block_coords(m, b, cb);
   const double xx = xcen(m, 0, cb[0], i);
@@ -159,19 +178,19 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
 #pragma unroll
   for (int r = 0; r < NW; ++r) {
 #pragma unroll
-    for (int v = 0; v < NV; ++v) cp_async8(&win[r][v][tid], src + v * m.ncell);
+    for (int v = 0; v < NQ; ++v) cp_async8(&win[r][v][tid], src + v * m.ncell);
     cp_async_commit();
     src += sd;
   }
   int s0 = 0;                                     // ring slot of row c-HW
   int snew = NW;                                  // ring slot the next prefetched row goes to
-  double qpPrev[NV];
+  double qpPrev[NQ];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) qpPrev[v] = 0.0;
+  for (int v = 0; v < NQ; ++v) qpPrev[v] = 0.0;
   for (int c = f0 - 1; c <= f1; ++c) {
     if (c + HW + 1 <= rlast) {
 #pragma unroll
-      for (int v = 0; v < NV; ++v) cp_async8(&win[snew][v][tid], src + v * m.ncell);
+      for (int v = 0; v < NQ; ++v) cp_async8(&win[snew][v][tid], src + v * m.ncell);
       src += sd;
     }
     cp_async_commit();
@@ -183,27 +202,32 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
       sl = (sl >= NR) ? sl - NR : sl;
       wrow[r] = &win[sl][0][tid];
     }
-    double qm[NV], qp[NV], centre[NV];
+    double qm[NQ], qp[NQ], centre[NQ];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) {
+    for (int v = 0; v < NQ; ++v) {
       double f[NW];
 #pragma unroll
       for (int r = 0; r < NW; ++r) f[r] = wrow[r][v * MS_BLOCK];
       centre[v] = f[HW];
       recon1<RECON>(f, qm[v], qp[v]);
     }
-    positivity_fallback<RECON>(m, centre, qm, qp);
+    {
+      double xc = 0.0;
+      if (RECON >= 3 && m.floor_form != 0) xc = xcen(m, D, cb[D], c);
+      if (D == 1) positivity_fallback<METRIC, RECON, NS>(m, xx, xc, xo, centre, qm, qp);
+      else positivity_fallback<METRIC, RECON, NS>(m, xx, xo, xc, centre, qm, qp);
+    }
     if (c >= f0) {
       Geo<METRIC> G;
       const double xf = xface(m, D, cb[D], c);
       if (D == 1) G.at(m, xx, xf, xo); else G.at(m, xx, xo, xf);
-      double F[NV];
-      face_flux<METRIC, D>(m, G, qpPrev, qm, F);
+      double F[NQ];
+      face_flux<METRIC, D, NS>(m, G, qpPrev, qm, F);
 #pragma unroll
-      for (int v = 0; v < NV; ++v) flux[col + v * m.ncell + (long long)c * sd] = F[v];
+      for (int v = 0; v < NQ; ++v) flux[col + v * m.ncell + (long long)c * sd] = F[v];
     }
 #pragma unroll
-    for (int v = 0; v < NV; ++v) qpPrev[v] = qp[v];
+    for (int v = 0; v < NQ; ++v) qpPrev[v] = qp[v];
     s0 = (s0 + 1 == NR) ? 0 : s0 + 1;
     snew = (snew + 1 == NR) ? 0 : snew + 1;
   }
@@ -231,7 +255,8 @@ __device__ __forceinline__ void ct_pair(const MeshDev& m, const FluxPtrs& fl, co
 
 // One cell of the update.  Returns sum_d max|lambda^d|/dx_d of the new primitives when CFL is set (0 for a thread without
 // a cell or with an excised one), so that the kernel can reduce the next time step on the fly.
-template <int METRIC, bool EXC, bool CFL>
+// RF: the floors depend on the position (floor_form != 0); a template flag so that the constant-floor kernels carry none of it
+template <int METRIC, bool EXC, bool CFL, int NS, bool RF>
 __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                               double bdt_host, const double* __restrict__ d_dt, double beta,
                                               const double* cons0, const double* cons_in, double* cons_out,
@@ -247,12 +272,13 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
   const int kk = blockIdx.y;
   const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
   const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
-  const long long vb = (long long)b * NV * m.ncell;     // block offset in an 8-variable field
+  constexpr int NQ = NV + NS;
+  const long long vb = (long long)b * m.nvar * m.ncell;  // block offset in a field of nvar variables
   const long long fb = (long long)b * m.ncell;          // block offset in a one-variable field
   if (EXC) {
     if (xfl[fb + c] & XF_CELL) {   // frozen cell: the RK combination of two equal states is exact
 #pragma unroll
-      for (int v = 0; v < NV; ++v) {
+      for (int v = 0; v < NQ; ++v) {
         const long long id = vb + v * m.ncell + c;
         cons_out[id] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] : cons0[id];
       }
@@ -262,15 +288,16 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
   }
   const double bdt = d_dt ? beta * (*d_dt) : bdt_host;
   const long long str[3] = {1, m.sj, m.sk};
-  double R[NV];
+  double R[NQ];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) R[v] = 0.0;
+  for (int v = 0; v < NQ; ++v) R[v] = 0.0;
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     if (!m.act[d]) continue;
     const double* F = fl.f[d] + vb + c;
 #pragma unroll
     for (int v = 0; v <= CTAU; ++v) R[v] -= (F[v * m.ncell + str[d]] - F[v * m.ncell]) * m.rdx[d];
+    if constexpr (NS == 1) R[XS] -= (F[XS * m.ncell + str[d]] - F[XS * m.ncell]) * m.rdx[d];   // no source: S = 0 in Eq.14
     // magnetic components that flux-CT does not replace (inactive partner direction, or CT switched off)
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc) {
@@ -289,7 +316,7 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
   int cb[3];
   block_coords(m, b, cb);
   const double x = xcen(m, 0, cb[0], i), y = xcen(m, 1, cb[1], j), z = xcen(m, 2, cb[2], k);
-  double U[NV], q[NV];
+  double U[NQ], q[NQ];
   // stage-input primitives of this cell: sources, and the initial guess of the con2prim root
   q[RHO] = prim[vb + RHO * m.ncell + c];
   q[UX] = prim[vb + UX * m.ncell + c]; q[UY] = prim[vb + UY * m.ncell + c]; q[UZ] = prim[vb + UZ * m.ncell + c];
@@ -301,21 +328,25 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
     R[CS1] += S[0]; R[CS2] += S[1]; R[CS3] += S[2]; R[CTAU] += S[3];
   }
 #pragma unroll
-  for (int v = 0; v < NV; ++v) {
+  for (int v = 0; v < NQ; ++v) {
     const long long id = vb + v * m.ncell + c;
     U[v] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] + bdt * R[v] : g0 * cons0[id] + bdt * R[v];
   }
   Geo<METRIC> G;
   G.at(m, x, y, z);
   const double mu_guess = c2p_guess<METRIC>(G, q, m.gam);
-  const unsigned char mk = c2p_cell<METRIC>(m, G, U, q, mu_guess);
+  double rfl = m.rho_floor, efl = m.eps_floor;
+  if constexpr (RF) floors_at<METRIC>(m, x, y, z, rfl, efl);
+  const double Dt_in = U[CD];
+  unsigned mk = c2p_cell<METRIC>(m, G, rfl, efl, U, q, mu_guess);
+  if constexpr (NS == 1) scalar_recover(m, Dt_in, U[CD], mk, U[XS], q[XS]);
 #pragma unroll
-  for (int v = 0; v < NV; ++v) {
+  for (int v = 0; v < NQ; ++v) {
     const long long id = vb + v * m.ncell + c;
     cons_out[id] = U[v];
     prim[id] = q[v];
   }
-  mask[fb + c] = mk;
+  mask[fb + c] = (unsigned char)mk;
   if constexpr (CFL) {
     double lam[3];
     max_speeds<METRIC>(q, G, m.gam, lam);
@@ -330,13 +361,13 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
 // smax: PHX_NSLOT accumulators of the largest sum_d max|lambda^d|/dx_d seen (bit pattern of a non-negative double, which
 // orders like the unsigned integer), one atomicMax per thread block; k_cfl_final_slots turns them into the time step.
 constexpr int PHX_NSLOT = 1024;
-template <int METRIC, bool EXC, bool CFL>
+template <int METRIC, bool EXC, bool CFL, int NS, bool RF>
 __global__ void __launch_bounds__(UP_BLOCK, (METRIC == 1 ? PHX_UP_MINB_KS : PHX_UP_MINB)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                                      double bdt_host, const double* __restrict__ d_dt, double beta,
                                                      const double* cons0, const double* cons_in, double* cons_out,
                                                      double* __restrict__ prim, unsigned char* __restrict__ mask,
                                                      unsigned long long* __restrict__ smax) {
-  double sum = update_cell<METRIC, EXC, CFL>(m, fl, xfl, g0, g1, bdt_host, d_dt, beta, cons0, cons_in, cons_out, prim, mask);
+  double sum = update_cell<METRIC, EXC, CFL, NS, RF>(m, fl, xfl, g0, g1, bdt_host, d_dt, beta, cons0, cons_in, cons_out, prim, mask);
   if constexpr (CFL) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum = fmax(sum, __shfl_xor_sync(0xffffffffu, sum, o));
@@ -371,7 +402,7 @@ __global__ void __launch_bounds__(256) k_cfl_final_slots(unsigned long long* __r
 }
 
 // ---- stand-alone con2prim, prim->cons ---------------------------------------------------------------
-template <int METRIC, bool EXC>
+template <int METRIC, bool EXC, int NS, bool RF>
 __global__ void __launch_bounds__(UP_BLOCK) k_c2p(MeshDev m, const unsigned char* __restrict__ xfl, double* __restrict__ cons,
                                                   double* __restrict__ prim, unsigned char* __restrict__ mask, long long ninterior) {
   const long long p = (long long)blockIdx.x * UP_BLOCK + threadIdx.x;
@@ -383,24 +414,30 @@ __global__ void __launch_bounds__(UP_BLOCK) k_c2p(MeshDev m, const unsigned char
   const int b = (int)(r / m.n[2]);
   const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
   const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
-  const long long vb = (long long)b * NV * m.ncell, fb = (long long)b * m.ncell;
+  constexpr int NQ = NV + NS;
+  const long long vb = (long long)b * m.nvar * m.ncell, fb = (long long)b * m.ncell;
   if (EXC) {
     if (xfl[fb + c] & XF_CELL) { mask[fb + c] = M_EXCISED; return; }
   }
   int cb[3];
   block_coords(m, b, cb);
   Geo<METRIC> G;
-  G.at(m, xcen(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
-  double U[NV], q[NV];
+  const double x = xcen(m, 0, cb[0], i), y = xcen(m, 1, cb[1], j), z = xcen(m, 2, cb[2], k);
+  G.at(m, x, y, z);
+  double U[NQ], q[NQ];
 #pragma unroll
-  for (int v = 0; v < NV; ++v) U[v] = cons[vb + v * m.ncell + c];
-  const unsigned char mk = c2p_cell<METRIC>(m, G, U, q);
+  for (int v = 0; v < NQ; ++v) U[v] = cons[vb + v * m.ncell + c];
+  double rfl = m.rho_floor, efl = m.eps_floor;
+  if constexpr (RF) floors_at<METRIC>(m, x, y, z, rfl, efl);
+  const double Dt_in = U[CD];
+  unsigned mk = c2p_cell<METRIC>(m, G, rfl, efl, U, q);
+  if constexpr (NS == 1) scalar_recover(m, Dt_in, U[CD], mk, U[XS], q[XS]);
 #pragma unroll
-  for (int v = 0; v < NV; ++v) {
-    if (mk & (M_RHO_FLOOR | M_EPS_FLOOR | M_W_CEIL | M_BAD_INPUT)) cons[vb + v * m.ncell + c] = U[v];
+  for (int v = 0; v < NQ; ++v) {
+    if (mk & (M_RHO_FLOOR | M_EPS_FLOOR | M_W_CEIL | M_BAD_INPUT | M_SCALAR_CLIPPED)) cons[vb + v * m.ncell + c] = U[v];
     prim[vb + v * m.ncell + c] = q[v];
   }
-  mask[fb + c] = mk;
+  mask[fb + c] = (unsigned char)mk;
 }
 
 template <int METRIC>
@@ -412,7 +449,7 @@ __global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* _
   const int j = (int)(r % m.na[1]); r /= m.na[1];
   const int k = (int)(r % m.na[2]);
   const int b = (int)(r / m.na[2]);
-  const long long id = (long long)b * NV * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
+  const long long id = (long long)b * m.nvar * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
   int cb[3];
   block_coords(m, b, cb);
   Geo<METRIC> G;
@@ -423,6 +460,7 @@ __global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* _
   prim_to_cons_pt<METRIC>(q, G, m.gam, U);
 #pragma unroll
   for (int v = 0; v < NV; ++v) cons[id + v * m.ncell] = U[v];
+  if (m.nvar > NV) cons[id + XS * m.ncell] = U[CD] * prim[id + XS * m.ncell];   // sqrt(gamma) D X (Eq.14)
 }
 
 // ---- ghost fill: one gather pass -------------------------------------------------------------------
@@ -459,13 +497,15 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restri
     sl[d] = li + m.g[d];
   }
   const int bs = (sb[2] * m.nb[1] + sb[1]) * m.nb[0] + sb[0];
-  const long long src = (long long)bs * NV * m.ncell + (long long)sl[2] * m.sk + (long long)sl[1] * m.sj + sl[0];
-  const long long dst = (long long)b * NV * m.ncell + (long long)l[2] * m.sk + (long long)l[1] * m.sj + l[0];
-  double v[NV];
+  const long long src = (long long)bs * m.nvar * m.ncell + (long long)sl[2] * m.sk + (long long)sl[1] * m.sj + sl[0];
+  const long long dst = (long long)b * m.nvar * m.ncell + (long long)l[2] * m.sk + (long long)l[1] * m.sj + l[0];
+  double v[NV + 1];
 #pragma unroll
   for (int q = 0; q < NV; ++q) v[q] = prim[src + q * m.ncell];
+  if (m.nvar > NV) v[XS] = prim[src + XS * m.ncell];
 #pragma unroll
   for (int q = 0; q < NV; ++q) prim[dst + q * m.ncell] = v[q];
+  if (m.nvar > NV) prim[dst + XS * m.ncell] = v[XS];
 }
 
 // ---- CFL: warp-shuffle min reduction ------------------------------------------------------------------
@@ -490,7 +530,7 @@ __global__ void __launch_bounds__(256) k_cfl_partial(MeshDev m, const unsigned c
     G.at(m, xcen(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
     double q[NV], lam[3];
 #pragma unroll
-    for (int v = 0; v < NV; ++v) q[v] = prim[(long long)b * NV * m.ncell + v * m.ncell + c];
+    for (int v = 0; v < NV; ++v) q[v] = prim[(long long)b * m.nvar * m.ncell + v * m.ncell + c];
     max_speeds<METRIC>(q, G, m.gam, lam);
     double s = 0.0;
 #pragma unroll
@@ -612,6 +652,11 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   if (!(p->rho_floor > 0.0) || !(p->eps_floor > 0.0) || !(p->w_max > 1.0)) return fail(PHX_EINVAL, "phx_init_mesh: floors must be positive, w_max > 1");
   if (!(p->c2p_tol > 0.0) || p->c2p_maxit < 1) return fail(PHX_EINVAL, "phx_init_mesh: c2p_tol > 0 and c2p_maxit >= 1 required");
   if (p->metric == PHX_KERR_SCHILD && !(p->bh_mass > 0.0)) return fail(PHX_EINVAL, "phx_init_mesh: bh_mass must be positive");
+  if (p->nscalar < 0 || p->nscalar > 1) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: nscalar must be 0 or 1");
+  if (p->nscalar == 1 && !(p->scalar_max > p->scalar_min)) return fail(PHX_EINVAL, "phx_init_mesh: scalar_max must exceed scalar_min");
+  if (p->floor_form < PHX_FLOOR_CONST || p->floor_form > PHX_FLOOR_POW_R) return fail(PHX_EUNSUPPORTED, "phx_init_mesh: unknown floor form");
+  if (p->floor_form != PHX_FLOOR_CONST && (!(p->floor_alpha_rho >= 0.0) || !(p->floor_alpha_eps >= 0.0)))
+    return fail(PHX_EINVAL, "phx_init_mesh: floor exponents must be non-negative");
   phx_mesh* M = new (std::nothrow) phx_mesh();
   if (!M) return fail(PHX_ENOMEM, "phx_init_mesh: host allocation failed");
   memset(M, 0, sizeof *M);
@@ -644,15 +689,18 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   m.rho_floor = p->rho_floor; m.eps_floor = p->eps_floor; m.w_max = p->w_max; m.c2p_tol = p->c2p_tol; m.c2p_maxit = p->c2p_maxit;
   m.excise = (p->metric == PHX_KERR_SCHILD && p->r_excise > 0.0) ? 1 : 0;
   for (int d = 0; d < 3; ++d) m.shift[d] = (p->metric == PHX_MINKOWSKI_BOOSTED) ? p->shift[d] : 0.0;
+  m.nvar = NV + p->nscalar;
+  m.xs_min = p->scalar_min; m.xs_max = p->scalar_max;
+  m.floor_form = p->floor_form; m.fl_arho = p->floor_alpha_rho; m.fl_aeps = p->floor_alpha_eps;
   M->nall = (long long)m.nblk * m.ncell;
   M->ninterior = (long long)m.nblk * m.n[0] * m.n[1] * m.n[2];
-  if (M->nall * NV >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
+  if (M->nall * m.nvar >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
   // launch geometry: blocks ride on gridDim.z, k-planes or sweep segments on gridDim.y (both limited to 65535)
   if (m.nblk > 65535 || m.na[2] > 65535 ||
       (long long)m.na[0] * m.na[1] >= (1LL << 31)) {
     delete M; return fail(PHX_EUNSUPPORTED, "phx_init_mesh: more than 65535 blocks or k-planes, or a k-plane of 2^31 cells");
   }
-  const size_t fbytes = (size_t)M->nall * NV * sizeof(double);
+  const size_t fbytes = (size_t)M->nall * m.nvar * sizeof(double);
   cudaStream_t st = (cudaStream_t)stream;
   for (int d = 0; d < 3; ++d) {
     if (!m.act[d]) continue;
@@ -690,12 +738,12 @@ extern "C" int phx_free_mesh(phx_mesh* M) {
   return PHX_OK;
 }
 
-extern "C" size_t phx_field_elems(const phx_mesh* M) { return M ? (size_t)M->nall * NV : 0; }
+extern "C" size_t phx_field_elems(const phx_mesh* M) { return M ? (size_t)M->nall * M->m.nvar : 0; }
 extern "C" size_t phx_mask_elems(const phx_mesh* M) { return M ? (size_t)M->nall : 0; }
 extern "C" unsigned long long phx_launch_count(const phx_mesh* M) { return M ? M->launches : 0; }
 extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* stream) {
   if (!M || d < 0 || d > 2 || !M->flux[d] || !aligned16(d_out)) return fail(PHX_EINVAL, "phx_debug_flux: null argument or inactive direction");
-  CUDA_TRY(cudaMemcpyAsync(d_out, M->flux[d], (size_t)M->nall * NV * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream), "cudaMemcpyAsync");
+  CUDA_TRY(cudaMemcpyAsync(d_out, M->flux[d], (size_t)M->nall * M->m.nvar * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream), "cudaMemcpyAsync");
   return PHX_OK;
 }
 
@@ -739,18 +787,25 @@ extern "C" int phx_cons_to_prim(const phx_mesh* Mc, double* d_cons, double* d_pr
   const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
   {
   ProfScope ps(M, PHX_K_C2P, st);
-#define CALL(MET)                                                                                         \
-  if (M->m.excise) k_c2p<MET, true><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior); \
-  else k_c2p<MET, false><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior)
+#define C2P(MET, EXC, NSC, RFL) k_c2p<MET, EXC, NSC, RFL><<<nb, UP_BLOCK, 0, st>>>(M->m, M->xfl, d_cons, d_prim, d_mask, M->ninterior)
+#define CALL(MET)                                                      \
+  if (M->m.nvar == NV) {                                               \
+    if (M->m.floor_form == 0) { if (M->m.excise) C2P(MET, true, 0, false); else C2P(MET, false, 0, false); } \
+    else { if (M->m.excise) C2P(MET, true, 0, true); else C2P(MET, false, 0, true); }                        \
+  } else {                                                             \
+    if (M->m.floor_form == 0) { if (M->m.excise) C2P(MET, true, 1, false); else C2P(MET, false, 1, false); } \
+    else { if (M->m.excise) C2P(MET, true, 1, true); else C2P(MET, false, 1, true); }                        \
+  }
   DISPATCH_METRIC(M, CALL);
 #undef CALL
+#undef C2P
   }
   LAUNCH_CHECK(M, "k_c2p");
   return phx_fill_ghosts(M, d_prim, stream);
 }
 
 // ---- sweeps -------------------------------------------------------------------------------------------------
-template <int METRIC, int RECON>
+template <int METRIC, int RECON, int NS>
 static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
   const MeshDev& m = M->m;
   int lo[3], cnt[3];
@@ -763,7 +818,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int nplane = cnt[1] * rowlen;
     dim3 grid((nplane + (XS_BLOCK - 2)) / (XS_BLOCK - 1), cnt[2], m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_X, st);
-    k_sweep_x<METRIC, RECON><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], nplane, rowlen, lo[1], lo[2]);
+    k_sweep_x<METRIC, RECON, NS><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], nplane, rowlen, lo[1], lo[2]);
     M->launches++;
   }
   const int Lmax = 33;
@@ -774,7 +829,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int ntr = cnt[0] * cnt[2];
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Y, st);
-    k_sweep_march<METRIC, RECON, 1><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], L);
+    k_sweep_march<METRIC, RECON, 1, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], L);
     M->launches++;
   }
   if (m.act[2]) {
@@ -784,7 +839,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int ntr = cnt[0] * cnt[1];
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Z, st);
-    k_sweep_march<METRIC, RECON, 2><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], L);
+    k_sweep_march<METRIC, RECON, 2, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], L);
     M->launches++;
   }
 }
@@ -792,7 +847,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
 static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
   const int key = M->m.metric * 6 + M->m.recon;
   switch (key) {
-#define PHX_CASE(MET, REC) case MET * 6 + REC: launch_sweeps_t<MET, REC>(M, prim, st); break;
+#define PHX_CASE(MET, REC) case MET * 6 + REC: if (M->m.nvar == NV) launch_sweeps_t<MET, REC, 0>(M, prim, st); else launch_sweeps_t<MET, REC, 1>(M, prim, st); break;
     PHX_CASE(0, 0) PHX_CASE(0, 1) PHX_CASE(0, 2) PHX_CASE(0, 3) PHX_CASE(0, 4) PHX_CASE(0, 5)
     PHX_CASE(1, 0) PHX_CASE(1, 1) PHX_CASE(1, 2) PHX_CASE(1, 3) PHX_CASE(1, 4) PHX_CASE(1, 5)
     PHX_CASE(2, 0) PHX_CASE(2, 1) PHX_CASE(2, 2) PHX_CASE(2, 3) PHX_CASE(2, 4) PHX_CASE(2, 5)
@@ -811,16 +866,17 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
   const dim3 nb((M->m.n[0] * M->m.n[1] + UP_BLOCK - 1) / UP_BLOCK, M->m.n[2], M->m.nblk);
   {
   ProfScope ps(M, PHX_K_UPDATE, st);
-#define CALL(MET)                                                                                                                   \
-  if (M->m.excise) { \
-    if (reduce_cfl) k_update<MET, true, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
-    else k_update<MET, true, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
-  } else { \
-    if (reduce_cfl) k_update<MET, false, true><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
-    else k_update<MET, false, false><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax); \
-  }
+#define UPD(MET, EXC, CFLR, NSC, RFL) k_update<MET, EXC, CFLR, NSC, RFL><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax)
+#define UPD2(MET, NSC, RFL)                                                                                  \
+  if (M->m.excise) { if (reduce_cfl) UPD(MET, true, true, NSC, RFL); else UPD(MET, true, false, NSC, RFL); } \
+  else { if (reduce_cfl) UPD(MET, false, true, NSC, RFL); else UPD(MET, false, false, NSC, RFL); }
+#define CALL(MET)                                                                    \
+  if (M->m.nvar == NV) { if (M->m.floor_form == 0) { UPD2(MET, 0, false) } else { UPD2(MET, 0, true) } } \
+  else { if (M->m.floor_form == 0) { UPD2(MET, 1, false) } else { UPD2(MET, 1, true) } }
   DISPATCH_METRIC(M, CALL);
 #undef CALL
+#undef UPD2
+#undef UPD
   }
   LAUNCH_CHECK(M, "k_update");
   return phx_fill_ghosts(M, d_prim, st);
@@ -920,7 +976,7 @@ extern "C" int phx_evolve_host(phx_mesh* M, const double* h_prim_in, int nsteps,
                                unsigned char* h_mask_out, double* h_t, void* stream) {
   if (!M || !h_prim_in || !h_prim_out || nsteps < 0 || !(cfl > 0.0)) return fail(PHX_EINVAL, "phx_evolve_host: null argument, nsteps < 0 or cfl <= 0");
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t fbytes = (size_t)M->nall * NV * sizeof(double);
+  const size_t fbytes = (size_t)M->nall * M->m.nvar * sizeof(double);
   if (!M->ws_scal) {
     for (int d = 0; d < 3; ++d)
       if (cudaMalloc((void**)&M->ws_field[d], fbytes) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }

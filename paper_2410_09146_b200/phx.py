@@ -38,16 +38,19 @@ class Params(C.Structure):
         ("gamma_ad", C.c_double), ("recon", C.c_int), ("riemann", C.c_int), ("use_ct", C.c_int),
         ("rho_floor", C.c_double), ("eps_floor", C.c_double), ("w_max", C.c_double),
         ("c2p_tol", C.c_double), ("c2p_maxit", C.c_int), ("shift", C.c_double * 3),
+        ("nscalar", C.c_int), ("scalar_min", C.c_double), ("scalar_max", C.c_double),
+        ("floor_form", C.c_int), ("floor_alpha_rho", C.c_double), ("floor_alpha_eps", C.c_double),
     ]
+
+# parameters added after the first version of the ABI: optional in the dictionaries, with the values that switch them off
+_OPTIONAL = dict(shift=(0.0, 0.0, 0.0), nscalar=0, scalar_min=0.0, scalar_max=1.0, floor_form=0,
+                 floor_alpha_rho=2.0, floor_alpha_eps=1.0)
 
 
 def make_params(p: dict) -> Params:
     q = Params()
     for name, _ in Params._fields_:
-        if name == "shift":
-            v = p.get("shift", (0.0, 0.0, 0.0))
-        else:
-            v = p[name]
+        v = p.get(name, _OPTIONAL[name]) if name in _OPTIONAL else p[name]
         if name in ("xmin", "xmax", "shift"):
             setattr(q, name, (C.c_double * 3)(*[float(t) for t in v]))
         elif name == "bc":
