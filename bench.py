@@ -65,7 +65,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n", type=int, default=256, help="zones per side of the config-4 box (256 = BASELINE.json)")
-    ap.add_argument("--workload", default="cfg4", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "next1", "next2"],
+    ap.add_argument("--workload", default="cfg4", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "next1", "next2", "next3"],
                     help="cfg4 (default) is the bench workload; the others time BASELINE.json's other 3-D configs at full size "
                          "(reported without a roofline object: the per-zone figures of DESIGN.md 6 are config 4's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -141,6 +141,8 @@ def make_workload(name, n):
         return wl.turbulence_box(n, recon=wl.RECON_WENO5Z_AOAH), f"next1_turbulence_box_{n}^3_weno5z_aoah_hll_ct_rk2_minkowski"
     if name == "next2":     # the paper's scaling workload shape, --n 128 is its size
         return wl.sedov_blast(n), f"next2_sedov_blast_{n}^3_plm_minmod_hll_rk2_minkowski"
+    if name == "next3":     # config 5 carrying a passive scalar (Eq.14) with the floors rho0 r^-2, eps0 r^-1
+        return _scalar_blocks(wl, (8, 8, 8)), "next3_packed_blocks_512x32^3_kerr_schild_passive_scalar_radial_floors"
     if name == "cfg1":
         return wl.shock_tube(256), "cfg1_shock_tube_256_plm_minmod_hll_rk2_minkowski"
     if name == "cfg2":
@@ -148,6 +150,12 @@ def make_workload(name, n):
     if name == "cfg3":
         return wl.kerr_schild_torus(128), "cfg3_kerr_schild_torus_128^3_plm_minmod_hll_ct_rk2"
     return wl.packed_blocks((8, 8, 8), 32), "cfg5_packed_blocks_512x32^3_kerr_schild_plm_minmod_hll_ct_rk2"
+
+
+def _scalar_blocks(wl, nb):
+    w = wl.packed_blocks(nb, 32)
+    w = dict(w, params=dict(w["params"], floor_form=3, rho_floor=1e-2, eps_floor=1e-2, floor_alpha_rho=2.0, floor_alpha_eps=1.0))
+    return wl.with_scalar(w, wl.smooth_scalar(w["params"], wl.SEED0 + 9))
 
 
 def oracle_sample(name):
@@ -159,6 +167,8 @@ def oracle_sample(name):
         return wl.turbulence_box(128, recon=wl.RECON_WENO5Z_AOAH), 3, "config-4 recipe with WENO5-Z-AOAH at 128^3, 3 RK2 steps"
     if name == "next2":
         return wl.sedov_blast(128), 3, "Sedov blast at 128^3, 3 RK2 steps"
+    if name == "next3":
+        return _scalar_blocks(wl, (4, 4, 4)), 2, "next3 recipe on 64 blocks of 32^3 (1/8 of the mesh), 2 RK2 steps"
     if name == "cfg1":
         return wl.shock_tube(256), 247, "the whole of config 1 (256 zones, 247 RK2 steps)"
     if name == "cfg2":

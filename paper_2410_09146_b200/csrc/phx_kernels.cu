@@ -44,6 +44,7 @@ constexpr int XS_BLOCK = PHX_XS_BLOCK;   // threads per block of the x sweep (XS
 constexpr int MS_BLOCK = PHX_MS_BLOCK;   // threads per block of the marching sweeps
 constexpr int UP_BLOCK = PHX_UP_BLOCK;
 
+
 // (x, y, z): centre of the cell, used only when the floors depend on the position (floor_form != 0)
 template <int METRIC, int RECON, int NS>
 __device__ __forceinline__ void positivity_fallback(const MeshDev& m, double x, double y, double z, const double* centre, double* qm,
@@ -464,19 +465,40 @@ __global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* _
 }
 
 // ---- ghost fill: one gather pass -------------------------------------------------------------------
-// blockIdx.z = block, blockIdx.y = allocated k-plane, the plane is tiled flat over (j, i); interior cells leave at once.
-__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim) {
-  const int p = blockIdx.x * 256 + threadIdx.x;
-  if (p >= m.na[0] * m.na[1]) return;
+// blockIdx.z = block; the threads enumerate the ghost cells of the block only: first the 2 g_z full k-planes, then the
+// 2 g_y full rows of every interior k-plane, then the 2 g_x end cells of every interior row (nA, nB: sizes of the first
+// two groups, ntot: all ghost cells of one block).
+__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, int nA, int nB, int ntot) {
+  int t = blockIdx.x * 256 + threadIdx.x;
+  if (t >= ntot) return;
   int l[3];
-  l[1] = p / m.na[0];
-  l[0] = p - l[1] * m.na[0];
-  l[2] = blockIdx.y;
+  if (t < nA) {
+    const int plane = m.na[0] * m.na[1];
+    const int kz = t / plane;
+    t -= kz * plane;
+    l[2] = kz < m.g[2] ? kz : kz + m.n[2];
+    l[1] = t / m.na[0];
+    l[0] = t - l[1] * m.na[0];
+  } else if (t < nA + nB) {
+    t -= nA;
+    const int per = 2 * m.g[1] * m.na[0];
+    const int kk = t / per;
+    t -= kk * per;
+    const int jy = t / m.na[0];
+    l[2] = m.g[2] + kk;
+    l[1] = jy < m.g[1] ? jy : jy + m.n[1];
+    l[0] = t - jy * m.na[0];
+  } else {
+    t -= nA + nB;
+    const int w = 2 * m.g[0];
+    const int row = t / w;
+    const int ix = t - row * w;
+    const int kk = row / m.n[1];
+    l[2] = m.g[2] + kk;
+    l[1] = m.g[1] + (row - kk * m.n[1]);
+    l[0] = ix < m.g[0] ? ix : ix + m.n[0];
+  }
   const int b = blockIdx.z;
-  bool interior = true;
-#pragma unroll
-  for (int d = 0; d < 3; ++d) interior = interior && (l[d] >= m.g[d]) && (l[d] < m.g[d] + m.n[d]);
-  if (interior) return;
   int cb[3], sb[3], sl[3];
   block_coords(m, b, cb);
 #pragma unroll
@@ -697,7 +719,7 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   if (M->nall * m.nvar >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
   // launch geometry: blocks ride on gridDim.z, k-planes or sweep segments on gridDim.y (both limited to 65535)
   if (m.nblk > 65535 || m.na[2] > 65535 ||
-      (long long)m.na[0] * m.na[1] >= (1LL << 31)) {
+      (long long)m.na[0] * m.na[1] >= (1LL << 31) || m.ncell >= (1LL << 31)) {
     delete M; return fail(PHX_EUNSUPPORTED, "phx_init_mesh: more than 65535 blocks or k-planes, or a k-plane of 2^31 cells");
   }
   const size_t fbytes = (size_t)M->nall * m.nvar * sizeof(double);
@@ -774,8 +796,10 @@ extern "C" int phx_fill_ghosts(const phx_mesh* Mc, double* d_prim, void* stream)
   if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
   if (M->nall == M->ninterior) return PHX_OK;
   { ProfScope ps(M, PHX_K_FILL_GHOSTS, (cudaStream_t)stream);
-    const dim3 grid((M->m.na[0] * M->m.na[1] + 255) / 256, M->m.na[2], M->m.nblk);
-    k_fill_ghosts<<<grid, 256, 0, (cudaStream_t)stream>>>(M->m, d_prim); }
+    const MeshDev& m = M->m;
+    const long long nA = 2LL * m.g[2] * m.na[1] * m.na[0], nB = 2LL * m.n[2] * m.g[1] * m.na[0], nC = 2LL * m.n[2] * m.n[1] * m.g[0];
+    const dim3 grid((unsigned)((nA + nB + nC + 255) / 256), 1, m.nblk);
+    k_fill_ghosts<<<grid, 256, 0, (cudaStream_t)stream>>>(m, d_prim, (int)nA, (int)nB, (int)(nA + nB + nC)); }
   LAUNCH_CHECK(M, "k_fill_ghosts");
   return PHX_OK;
 }

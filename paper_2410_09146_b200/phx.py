@@ -16,7 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libphx.so")
 
 OK, EINVAL, ECUDA, ENOMEM, EUNSUPPORTED = 0, 1, 2, 3, 4
-M_RHO_FLOOR, M_EPS_FLOOR, M_EPS_CLIPPED, M_W_CEIL, M_NOCONV, M_BAD_INPUT, M_EXCISED = 1, 2, 4, 8, 16, 32, 64
+M_RHO_FLOOR, M_EPS_FLOOR, M_EPS_CLIPPED, M_W_CEIL, M_NOCONV, M_BAD_INPUT, M_EXCISED, M_SCALAR_CLIPPED = 1, 2, 4, 8, 16, 32, 64, 128
+FLOOR_CONST, FLOOR_EXP_X1, FLOOR_POW_X1, FLOOR_POW_R = 0, 1, 2, 3
 
 KERNEL_CLASSES = ("sweep_x", "sweep_y", "sweep_z", "update", "fill_ghosts", "cfl", "prim_to_cons", "c2p", "copy")
 
