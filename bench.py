@@ -46,16 +46,16 @@ ALGO_BYTES_PER_ZONE = {
 # fp64 flop per interior zone and launch for the WENO5-Z + HLL Minkowski path: dadd + dmul + 2*dfma thread-instructions of
 # the committed kernels counted by ncu (profiles/r01_ncu_summary.md; con2prim iterations are data dependent, the figure
 # is the one measured on this workload).  achieved = these flops / measured time, i.e. useful fp64 work only.
-# update: average of the first stage (671) and the second stage, which also evaluates the signal speeds for the fused CFL
-# reduction (800); the "cfl" class is the one-block final kernel of that reduction
-ALGO_FLOP_PER_ZONE = {"sweep_x": 1328.0, "sweep_y": 1346.0, "sweep_z": 1346.0, "update": 736.0, "cfl": 0.0}
+# update: average of the first stage (670) and the second stage, which also evaluates the signal speeds for the fused CFL
+# reduction (798); the "cfl" class is the one-block final kernel of that reduction
+ALGO_FLOP_PER_ZONE = {"sweep_x": 1071.0, "sweep_y": 1085.0, "sweep_z": 1085.0, "update": 734.0, "cfl": 0.0}
 # fp64 peak from unit counts and clocks: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz; a DFMA loop measured
 # 33.9 TFLOP/s on this pool's B200 (16.94 T DFMA/s)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 FP64_MEASURED_DFMA_TFLOPS = 33.9
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (bytes)
-NCU_TRAFFIC = {256: {"update": 7.78e9, "sweep_x": 2.207e9, "sweep_y": 2.295e9, "sweep_z": 2.293e9, "cfl": 0.0,
-                     "fill_ghosts": 0.236e9}}
+NCU_TRAFFIC = {256: {"update": 7.725e9, "sweep_x": 2.206e9, "sweep_y": 2.304e9, "sweep_z": 2.301e9, "cfl": 0.0,
+                     "fill_ghosts": 0.256e9}}
 
 
 def parse_args():

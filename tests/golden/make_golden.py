@@ -50,7 +50,38 @@ def one_step_checksums():
     return out
 
 
+def next3_workloads():
+    """passive scalar (Eq.14) and the floors rho0 r^-2, eps0 r^-1."""
+    fl = dict(floor_form=3, rho_floor=1e-2, eps_floor=1e-2, floor_alpha_rho=2.0, floor_alpha_eps=1.0)
+    def scalar(w, seed):
+        return wl.with_scalar(w, wl.smooth_scalar(w["params"], seed))
+    def floors(w):
+        return dict(w, params=dict(w["params"], **fl))
+    return (("next3_turb_16_scalar", scalar(wl.turbulence_box(16), 1)),
+            ("next3_ks_torus_16_scalar_rfloor", scalar(floors(wl.kerr_schild_torus(16)), 2)),
+            ("next3_blocks_2x2x2_of_8_scalar_rfloor", scalar(floors(wl.packed_blocks((2, 2, 2), 8)), 3)))
+
+
+def next3_checksums():
+    out = []
+    for name, w in next3_workloads():
+        p = w["params"]
+        o = orc.Run(p, w["prim"])
+        dt = o.dt(w["cfl"])
+        o.step(dt)
+        c = wl.from_blocks(p, o.cons).reshape(9, -1)
+        m = wl.from_blocks(p, o.mask[:, None])[0]
+        out.append((name, dt, c.sum(axis=1), (c * c).sum(axis=1), [int(((m & b) != 0).sum()) for b in (1, 2, 64, 128)]))
+    return out
+
+
 if __name__ == "__main__":
+    with open(os.path.join(HERE, "one_step_checksums_next3.txt"), "w") as f:
+        f.write("# oracle, one RK2 step at CFL 0.4 of small workloads with the passive scalar / radial floors; written by tests/golden/make_golden.py\n")
+        f.write("# name dt  sum(U~_v) v=0..8  sum(U~_v^2) v=0..8  cells with mask bit 1, 2, 64, 128 after stage 2\n")
+        for name, dt, s1, s2, bits in next3_checksums():
+            f.write(name + " " + "%.15e " % dt + " ".join("%.15e" % v for v in s1) + " " + " ".join("%.15e" % v for v in s2)
+                    + " " + " ".join(str(b) for b in bits) + "\n")
     nsteps, rows = shock_tube_profile()
     with open(os.path.join(HERE, "cfg1_shock_tube_t0.4.txt"), "w") as f:
         f.write("# oracle, BASELINE.json configs[0]: 256 zones, PLM-minmod, HLL, RK2, CFL 0.4, t = 0.4; %d steps\n" % nsteps)

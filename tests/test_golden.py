@@ -31,12 +31,35 @@ def read_checksums():
     return out
 
 
+def _next3():
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(GOLD, "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    return dict(mod.next3_workloads())
+
+
+def read_next3():
+    out = {}
+    with open(os.path.join(GOLD, "one_step_checksums_next3.txt")) as f:
+        for line in f:
+            if line.startswith("#"):
+                continue
+            t = line.split()
+            v = np.array([float(x) for x in t[1:20]])
+            out[t[0]] = (v[0], v[1:10], v[10:19], [int(x) for x in t[20:24]])
+    return out
+
+
+NEXT3 = ("next3_turb_16_scalar", "next3_ks_torus_16_scalar_rfloor", "next3_blocks_2x2x2_of_8_scalar_rfloor")
+
+
 def read_shock_tube():
     return np.loadtxt(os.path.join(GOLD, "cfg1_shock_tube_t0.4.txt"))
 
 
 def check_sums(c, s1, s2, tol):
-    c = c.reshape(8, -1)
+    c = c.reshape(len(s1), -1)
     scale = np.sqrt(s2.max() * c.shape[1])                 # a sum of N terms of the largest variable's size
     assert np.abs(c.sum(axis=1) - s1).max() <= tol * scale
     assert np.abs((c * c).sum(axis=1) - s2).max() <= tol * s2.max()
@@ -51,6 +74,19 @@ def test_oracle_reproduces_stored_one_step_checksums(name):
     assert abs(o.dt(w["cfl"]) - dt) <= 1e-14 * dt
     o.step(dt)
     check_sums(wl.from_blocks(p, o.cons), s1, s2, 1e-13)
+
+
+@pytest.mark.parametrize("name", NEXT3)
+def test_oracle_reproduces_stored_next3_checksums(name):
+    dt, s1, s2, bits = read_next3()[name]
+    w = _next3()[name]
+    p = w["params"]
+    o = orc.Run(p, w["prim"])
+    assert abs(o.dt(w["cfl"]) - dt) <= 1e-14 * dt
+    o.step(dt)
+    check_sums(wl.from_blocks(p, o.cons), s1, s2, 1e-13)
+    m = wl.from_blocks(p, o.mask[:, None])[0]
+    assert [int(((m & b) != 0).sum()) for b in (1, 2, 64, 128)] == bits
 
 
 def test_oracle_reproduces_stored_shock_tube_profile():
@@ -77,6 +113,22 @@ def test_gpu_reproduces_stored_one_step_checksums(name):
     assert abs(g.dt(w["cfl"]) - dt) <= 1e-13 * dt
     g.step(dt)
     check_sums(wl.from_blocks(p, g.get()[0]), s1, s2, 1e-11)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("name", NEXT3)
+def test_gpu_reproduces_stored_next3_checksums(name):
+    from harness import GpuRun
+    dt, s1, s2, bits = read_next3()[name]
+    w = _next3()[name]
+    p = w["params"]
+    g = GpuRun(p, w["prim"])
+    assert abs(g.dt(w["cfl"]) - dt) <= 1e-13 * dt
+    g.step(dt)
+    cons, _, _, mask = g.get()
+    check_sums(wl.from_blocks(p, cons), s1, s2, 1e-11)
+    m = wl.from_blocks(p, mask[:, None])[0]
+    assert [int(((m & b) != 0).sum()) for b in (1, 2, 64, 128)] == bits
 
 
 @pytest.mark.gpu

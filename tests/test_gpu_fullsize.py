@@ -97,7 +97,8 @@ def run_full(w, origins, check_conservation):
     assert not (mask & (16 | 32)).any(), "con2prim failure bits at full size"
     cg = wl.from_blocks(p, cons)
     mg = wl.from_blocks(p, mask[:, None])[0]
-    scale = np.abs(cg).reshape(8, -1).max(axis=1)
+    nv = cg.shape[0]
+    scale = np.abs(cg).reshape(nv, -1).max(axis=1)
     scale = np.where(scale > 0.0, scale, 1.0)          # B = 0 workloads
     ddiv = np.abs(corner_div(cg[5:8], rdx) - div0).max()
     bscale = np.abs(c0[5:8]).max() * max(rdx)
@@ -106,7 +107,7 @@ def run_full(w, origins, check_conservation):
         rel = np.abs(np.sum(cg - c0, axis=(1, 2, 3), dtype=np.longdouble)) / np.sum(np.abs(c0), axis=(1, 2, 3))
         assert rel.max() <= 1e-13, f"totals drifted by {rel}"
     del c0, div0
-    worst = np.zeros(8)
+    worst = np.zeros(nv)
     for origin in origins:
         ps, sprim = sub_box(p, q_glob, origin)
         orc.reset_c2p_margin()
@@ -119,7 +120,7 @@ def run_full(w, origins, check_conservation):
         gi = [np.arange(origin[d] + vr[d].start, origin[d] + vr[d].stop) % N[d] for d in range(3)]
         got = cg[:, gi[2]][:, :, gi[1]][:, :, :, gi[0]]
         gm = mg[gi[2]][:, gi[1]][:, :, gi[0]]
-        err = np.abs(got - oc[sl_sub]).reshape(8, -1).max(axis=1) / scale
+        err = np.abs(got - oc[sl_sub]).reshape(nv, -1).max(axis=1) / scale
         worst = np.maximum(worst, err)
         assert err.max() <= TOL_1STEP, f"sub-box at {origin}: errors {err}"
         assert np.array_equal(gm, om[sl_sub[1:]]), f"sub-box at {origin}: masks differ"
@@ -173,3 +174,14 @@ def test_next2_sedov_128_sampled():
     w = wl.sedov_blast(128)
     n, s = 128, CORE + 2 * HALO
     run_full(w, [(48, 48, 48), (0, 0, 0), (n - s, 40, 60), (56, 60, 44)], check_conservation=False)
+
+
+def test_next3_packed_blocks_scalar_radial_floors_sampled():
+    """SURVEY.md 8(f) rank 3 at config 5's size: 512 blocks of 32^3 carrying the passive scalar of Eq.14 with the floors
+    rho0 r^-2, eps0 r^-1; nine variables and the masks (floor bits near the hole, excision) on sub-boxes
+    around the hole, at a domain corner and across block corners."""
+    w = wl.packed_blocks((8, 8, 8), 32)
+    w = dict(w, params=dict(w["params"], floor_form=3, rho_floor=1e-2, eps_floor=1e-2, floor_alpha_rho=2.0, floor_alpha_eps=1.0))
+    w = wl.with_scalar(w, wl.smooth_scalar(w["params"], wl.SEED0 + 9))
+    n, s = 256, CORE + 2 * HALO
+    run_full(w, [(112, 112, 112), (0, 0, 0), (n - s, n - s, n - s), (100, 120, 90), (176, 16, 208)], check_conservation=False)
