@@ -845,12 +845,23 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     k_sweep_x<METRIC, RECON, NS><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], nplane, rowlen, lo[1], lo[2]);
     M->launches++;
   }
-  const int Lmax = 33;
+  // Segments of at most 33 faces along the sweep direction; a small mesh gets more, shorter segments (at least 4 faces)
+  // until the launch has about four waves of thread blocks, so that the marching sweeps do not starve for parallelism
+  // (64^3: 2 segments = 0.9 blocks per SM -> 17 segments).  The fluxes do not depend on the segmentation.
+  auto segments = [&](int nfaces, int ntr) {
+    int nseg = (nfaces + 32) / 33;
+    const long long per_seg = (long long)((ntr + MS_BLOCK - 1) / MS_BLOCK) * m.nblk;
+    const long long want = 148LL * PHX_MS_MINB * 4;
+    const int need = (int)((want + per_seg - 1) / per_seg);
+    const int cap = (nfaces + 3) / 4;
+    if (need > nseg) nseg = need < cap ? need : cap;
+    return nseg < 1 ? 1 : nseg;
+  };
   if (m.act[1]) {
     const int nfaces = m.n[1] + 1;
-    const int nseg = (nfaces + Lmax - 1) / Lmax;
-    const int L = (nfaces + nseg - 1) / nseg;
     const int ntr = cnt[0] * cnt[2];
+    const int nseg = segments(nfaces, ntr);
+    const int L = (nfaces + nseg - 1) / nseg;
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Y, st);
     k_sweep_march<METRIC, RECON, 1, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], L);
@@ -858,9 +869,9 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
   }
   if (m.act[2]) {
     const int nfaces = m.n[2] + 1;
-    const int nseg = (nfaces + Lmax - 1) / Lmax;
-    const int L = (nfaces + nseg - 1) / nseg;
     const int ntr = cnt[0] * cnt[1];
+    const int nseg = segments(nfaces, ntr);
+    const int L = (nfaces + nseg - 1) / nseg;
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Z, st);
     k_sweep_march<METRIC, RECON, 2, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], L);
