@@ -43,6 +43,9 @@ using namespace phx;
 constexpr int XS_BLOCK = PHX_XS_BLOCK;   // threads per block of the x sweep (XS_BLOCK-1 faces per block)
 constexpr int MS_BLOCK = PHX_MS_BLOCK;   // threads per block of the marching sweeps
 constexpr int UP_BLOCK = PHX_UP_BLOCK;
+#ifndef PHX_UP_STAGE_KS
+#define PHX_UP_STAGE_KS 1  // Kerr-Schild update: U~0, U~_in and the stage-input primitives go through cp.async (2.42 -> 2.38 ms on
+#endif                     // 512 blocks of 32^3); the flat-metric update loses L1 capacity to it (1.51 -> 1.61 ms at 256^3): off there
 
 
 // (x, y, z): centre of the cell, used only when the floors depend on the position (floor_form != 0)
@@ -287,6 +290,27 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
       return 0.0;
     }
   }
+  // Kerr-Schild only (see PHX_UP_STAGE_KS): the cell's own streaming operands (U~0, U~_in, stage-input primitives) are fetched
+  // by cp.async into shared memory before the flux phase: they are in flight while the flux / CT loads go out and cost no
+  // registers until they are used.
+  // Every thread reads back only what it copied itself, so cp.async.wait_group is all the synchronisation needed.
+  constexpr int STG = (METRIC == 1) ? PHX_UP_STAGE_KS : 0;
+  constexpr int NPQ = (METRIC == 1) ? NV : 5;
+  __shared__ double stg[STG ? (2 * NQ + (STG == 1 ? NPQ : 0)) : 1][UP_BLOCK];
+  const int tid = threadIdx.x;
+  if constexpr (STG != 0) {
+#pragma unroll
+    for (int v = 0; v < NQ; ++v) cp_async8(&stg[v][tid], cons0 + vb + v * m.ncell + c);
+    if (g1 != 0.0) {
+#pragma unroll
+      for (int v = 0; v < NQ; ++v) cp_async8(&stg[NQ + v][tid], cons_in + vb + v * m.ncell + c);
+    }
+    if constexpr (STG == 1) {
+#pragma unroll
+      for (int v = 0; v < NPQ; ++v) cp_async8(&stg[2 * NQ + v][tid], prim + vb + v * m.ncell + c);
+    }
+    cp_async_commit();
+  }
   const double bdt = d_dt ? beta * (*d_dt) : bdt_host;
   const long long str[3] = {1, m.sj, m.sk};
   double R[NQ];
@@ -319,19 +343,26 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
   const double x = xcen(m, 0, cb[0], i), y = xcen(m, 1, cb[1], j), z = xcen(m, 2, cb[2], k);
   double U[NQ], q[NQ];
   // stage-input primitives of this cell: sources, and the initial guess of the con2prim root
-  q[RHO] = prim[vb + RHO * m.ncell + c];
-  q[UX] = prim[vb + UX * m.ncell + c]; q[UY] = prim[vb + UY * m.ncell + c]; q[UZ] = prim[vb + UZ * m.ncell + c];
-  q[UU] = prim[vb + UU * m.ncell + c];
+  if constexpr (STG != 0) cp_async_wait<0>();
+  if constexpr (STG == 1) {
+#pragma unroll
+    for (int v = 0; v < NPQ; ++v) q[v] = stg[2 * NQ + v][tid];
+  } else {
+    q[RHO] = prim[vb + RHO * m.ncell + c];
+    q[UX] = prim[vb + UX * m.ncell + c]; q[UY] = prim[vb + UY * m.ncell + c]; q[UZ] = prim[vb + UZ * m.ncell + c];
+    q[UU] = prim[vb + UU * m.ncell + c];
+    if constexpr (METRIC == 1) { q[BX] = prim[vb + BX * m.ncell + c]; q[BY] = prim[vb + BY * m.ncell + c]; q[BZ] = prim[vb + BZ * m.ncell + c]; }
+  }
   if constexpr (METRIC == 1) {
     double S[4];
-    q[BX] = prim[vb + BX * m.ncell + c]; q[BY] = prim[vb + BY * m.ncell + c]; q[BZ] = prim[vb + BZ * m.ncell + c];
     ks_sources(m, x, y, z, q, S);
     R[CS1] += S[0]; R[CS2] += S[1]; R[CS3] += S[2]; R[CTAU] += S[3];
   }
 #pragma unroll
   for (int v = 0; v < NQ; ++v) {
     const long long id = vb + v * m.ncell + c;
-    U[v] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] + bdt * R[v] : g0 * cons0[id] + bdt * R[v];
+    if constexpr (STG != 0) U[v] = (g1 != 0.0) ? g0 * stg[v][tid] + g1 * stg[NQ + v][tid] + bdt * R[v] : g0 * stg[v][tid] + bdt * R[v];
+    else U[v] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] + bdt * R[v] : g0 * cons0[id] + bdt * R[v];
   }
   Geo<METRIC> G;
   G.at(m, x, y, z);
