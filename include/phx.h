@@ -119,9 +119,18 @@ int phx_rk2_step(phx_mesh* mesh, const double* d_dt, double* d_cons0, double* d_
 int phx_rk2_step_cfl(phx_mesh* mesh, double cfl, double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
                      unsigned char* d_mask, void* stream);
 
+/* `nsteps` RK2 steps with the time step kept on the device: the same bits as `nsteps` calls of phx_rk2_step_cfl (*d_dt on
+ * entry = the time step of the first step, e.g. from phx_cfl_dt; on return = the CFL time step of the final state).
+ * d_t (DEVICE, nullable): the dt of every step is added to it before the step is taken (elapsed coordinate time).
+ * For nsteps >= 2 and no per-kernel timing active, the launches of one step are captured once into a CUDA graph (cached in
+ * the mesh for this set of arguments) and replayed on a mesh-owned stream fenced by events against `stream`, which removes
+ * the launch gaps that dominate small meshes (256 zones: 11 launches of a few microseconds per step).  Asynchronous. */
+int phx_evolve_device(phx_mesh* mesh, int nsteps, double cfl, double* d_dt, double* d_t, double* d_cons0, double* d_cons,
+                      double* d_prim, unsigned char* d_mask, void* stream);
+
 /* HOST-buffer path (the end-to-end call): copies h_prim_in (HOST, phx_field_elems doubles, ghosts filled) to
- * mesh-owned device fields, computes U~ (phx_prim_to_cons), then runs phx_cfl_dt once and `nsteps` times phx_rk2_step_cfl
- * with the time step kept on the device, and copies the primitives (required), the conserved variables and the
+ * mesh-owned device fields, computes U~ (phx_prim_to_cons), then runs phx_cfl_dt once and phx_evolve_device for `nsteps` steps
+ * (the time step kept on the device), and copies the primitives (required), the conserved variables and the
  * last stage's mask (both nullable) back to HOST buffers.  *h_t (nullable) receives the elapsed coordinate time.
  * Synchronises `stream` before returning.  The device workspace (3 fields + mask) is allocated on first use and
  * freed with the mesh.  Pinned host buffers make the copies asynchronous-capable but are not required. */

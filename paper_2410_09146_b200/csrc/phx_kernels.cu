@@ -18,7 +18,9 @@
 using namespace phx;
 
 // ================================================================================================ kernels
-// launch shapes (tuned on B200 with ncu, profiles/): threads per block and minimum resident blocks per SM
+// launch shapes (tuned on B200 with ncu, profiles/): threads per block and minimum resident blocks per SM; the x sweep is
+// bound to 6 blocks/SM for WENO5-Z-AOAH and to 5 for Kerr-Schild with PLM (96 registers, no spills: 0.90 -> 0.83 ms on
+// 512 blocks of 32^3), WENO5-Z keeps its 128 registers (more blocks per SM measured slower there)
 #ifndef PHX_XS_BLOCK
 #define PHX_XS_BLOCK 128
 #endif
@@ -80,7 +82,7 @@ __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G
 // ---- x sweep ------------------------------------------------------------------------------------
 // position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
 template <int METRIC, int RECON, int NS>
-__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : PHX_XS_MINB)) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : (METRIC == 1 && RECON <= 2 ? 5 : PHX_XS_MINB))) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
                                                       int nplane, int rowlen, int j0, int k0) {
   // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii)
   constexpr int HW = ReconTraits<RECON>::HW;
@@ -663,6 +665,12 @@ struct phx_mesh {
   cudaEvent_t* ev;   // 2 events per recorded launch
   int* evcls;
   int evcap, evn;
+  // CUDA graph of one RK2 step (phx_evolve_device): captured once per argument set on a mesh-owned stream and replayed
+  cudaStream_t gstream;
+  cudaEvent_t gev_in, gev_out;
+  cudaGraphExec_t gexec;
+  unsigned long long glaunches;        // kernel launches one replay stands for
+  struct { double cfl; double *dt, *t, *cons0, *cons, *prim; unsigned char* mask; } gkey;
 };
 
 // RAII pair of events around one launch (or one group of launches) of class `cls`, recorded on the launching stream
@@ -787,6 +795,10 @@ extern "C" int phx_free_mesh(phx_mesh* M) {
   if (M->ws_mask) cudaFree(M->ws_mask);
   if (M->ws_scal) cudaFree(M->ws_scal);
   if (M->ev) { for (int i = 0; i < 2 * M->evcap; ++i) cudaEventDestroy(M->ev[i]); delete[] M->ev; delete[] M->evcls; }
+  if (M->gexec) cudaGraphExecDestroy(M->gexec);
+  if (M->gev_in) cudaEventDestroy(M->gev_in);
+  if (M->gev_out) cudaEventDestroy(M->gev_out);
+  if (M->gstream) cudaStreamDestroy(M->gstream);
   delete M;
   return PHX_OK;
 }
@@ -1036,7 +1048,66 @@ extern "C" int phx_profile_read(phx_mesh* M, double* h_ms, unsigned long long* h
 }
 
 // ---- host-buffer path ------------------------------------------------------------------------------------------
-__global__ void k_accumulate_time(double* __restrict__ scal) { scal[1] += scal[0]; }
+__global__ void k_accumulate_time(double* __restrict__ t, const double* __restrict__ dt) { *t += *dt; }
+
+// One step of phx_evolve_device: t += dt (before the step replaces dt), then phx_rk2_step_cfl.
+static int evolve_one(phx_mesh* M, double cfl, double* d_dt, double* d_t, double* d_cons0, double* d_cons, double* d_prim,
+                      unsigned char* d_mask, cudaStream_t st) {
+  if (d_t) {
+    k_accumulate_time<<<1, 1, 0, st>>>(d_t, d_dt);
+    LAUNCH_CHECK(M, "k_accumulate_time");
+  }
+  return phx_rk2_step_cfl(M, cfl, d_dt, d_cons0, d_cons, d_prim, d_mask, st);
+}
+
+extern "C" int phx_evolve_device(phx_mesh* M, int nsteps, double cfl, double* d_dt, double* d_t, double* d_cons0, double* d_cons,
+                                 double* d_prim, unsigned char* d_mask, void* stream) {
+  if (!M || nsteps < 0 || !d_dt || !(cfl > 0.0) || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask || d_cons0 == d_cons)
+    return fail(PHX_EINVAL, "phx_evolve_device: null, misaligned or aliased argument, nsteps < 0 or cfl <= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  if (nsteps == 0) return PHX_OK;
+  // per-kernel timing records events around every launch, which a replayed graph cannot serve: launch directly then
+  if (M->ev || nsteps < 2) {
+    for (int s = 0; s < nsteps; ++s) {
+      const int rc = evolve_one(M, cfl, d_dt, d_t, d_cons0, d_cons, d_prim, d_mask, st);
+      if (rc != PHX_OK) return rc;
+    }
+    return PHX_OK;
+  }
+  if (!M->gstream) {
+    CUDA_TRY(cudaStreamCreateWithFlags(&M->gstream, cudaStreamNonBlocking), "cudaStreamCreateWithFlags");
+    CUDA_TRY(cudaEventCreateWithFlags(&M->gev_in, cudaEventDisableTiming), "cudaEventCreateWithFlags");
+    CUDA_TRY(cudaEventCreateWithFlags(&M->gev_out, cudaEventDisableTiming), "cudaEventCreateWithFlags");
+  }
+  const bool same = M->gexec && M->gkey.cfl == cfl && M->gkey.dt == d_dt && M->gkey.t == d_t && M->gkey.cons0 == d_cons0 &&
+                    M->gkey.cons == d_cons && M->gkey.prim == d_prim && M->gkey.mask == d_mask;
+  if (!same) {
+    if (M->gexec) { cudaGraphExecDestroy(M->gexec); M->gexec = nullptr; }
+    // capture on the mesh-owned stream (the caller's may be the legacy default stream, which cannot be captured)
+    const unsigned long long before = M->launches;
+    CUDA_TRY(cudaStreamBeginCapture(M->gstream, cudaStreamCaptureModeThreadLocal), "cudaStreamBeginCapture");
+    const int rc = evolve_one(M, cfl, d_dt, d_t, d_cons0, d_cons, d_prim, d_mask, M->gstream);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(M->gstream, &graph);
+    M->glaunches = M->launches - before;
+    M->launches = before;                              // nothing ran during the capture
+    if (rc != PHX_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture");
+    const cudaError_t ei = cudaGraphInstantiate(&M->gexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (ei != cudaSuccess) { M->gexec = nullptr; return cuda_fail(ei, "cudaGraphInstantiate"); }
+    M->gkey.cfl = cfl; M->gkey.dt = d_dt; M->gkey.t = d_t; M->gkey.cons0 = d_cons0; M->gkey.cons = d_cons; M->gkey.prim = d_prim;
+    M->gkey.mask = d_mask;
+  }
+  // fence the mesh-owned stream behind the caller's stream, replay, fence the caller's stream behind the replays
+  CUDA_TRY(cudaEventRecord(M->gev_in, st), "cudaEventRecord");
+  CUDA_TRY(cudaStreamWaitEvent(M->gstream, M->gev_in, 0), "cudaStreamWaitEvent");
+  for (int s = 0; s < nsteps; ++s) CUDA_TRY(cudaGraphLaunch(M->gexec, M->gstream), "cudaGraphLaunch");
+  M->launches += M->glaunches * (unsigned long long)nsteps;
+  CUDA_TRY(cudaEventRecord(M->gev_out, M->gstream), "cudaEventRecord");
+  CUDA_TRY(cudaStreamWaitEvent(st, M->gev_out, 0), "cudaStreamWaitEvent");
+  return PHX_OK;
+}
 
 extern "C" int phx_evolve_host(phx_mesh* M, const double* h_prim_in, int nsteps, double cfl, double* h_prim_out, double* h_cons_out,
                                unsigned char* h_mask_out, double* h_t, void* stream) {
@@ -1061,12 +1132,8 @@ extern "C" int phx_evolve_host(phx_mesh* M, const double* h_prim_in, int nsteps,
     rc = phx_cfl_dt(M, prim, cfl, M->ws_scal, nullptr, st);
     if (rc != PHX_OK) return rc;
   }
-  for (int s = 0; s < nsteps; ++s) {
-    k_accumulate_time<<<1, 1, 0, st>>>(M->ws_scal);      // t += dt of this step, before the step replaces dt
-    LAUNCH_CHECK(M, "k_accumulate_time");
-    rc = phx_rk2_step_cfl(M, cfl, M->ws_scal, cons0, cons, prim, M->ws_mask, st);
-    if (rc != PHX_OK) return rc;
-  }
+  rc = phx_evolve_device(M, nsteps, cfl, M->ws_scal, M->ws_scal + 1, cons0, cons, prim, M->ws_mask, st);   // t += dt, step; graph replay
+  if (rc != PHX_OK) return rc;
   CUDA_TRY(cudaMemcpyAsync(h_prim_out, prim, fbytes, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
   if (h_cons_out) CUDA_TRY(cudaMemcpyAsync(h_cons_out, cons, fbytes, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");
   if (h_mask_out) CUDA_TRY(cudaMemcpyAsync(h_mask_out, M->ws_mask, (size_t)M->nall, cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync D2H");

@@ -25,7 +25,7 @@ EXPORTS = (
     "phx_init_mesh", "phx_free_mesh", "phx_field_elems", "phx_mask_elems", "phx_prim_to_cons",
     "phx_cons_to_prim", "phx_fill_ghosts", "phx_rk_stage", "phx_cfl_dt", "phx_rk2_step",
     "phx_evolve_host", "phx_debug_flux", "phx_launch_count", "phx_last_error",
-    "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl",
+    "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl", "phx_evolve_device",
 )
 
 
@@ -92,6 +92,7 @@ def lib():
         L.phx_cfl_dt.argtypes = [vp, dp, C.c_double, dp, C.POINTER(C.c_double), vp]
         L.phx_rk2_step.argtypes = [vp, dp, dp, dp, dp, ucp, vp]
         L.phx_rk2_step_cfl.argtypes = [vp, C.c_double, dp, dp, dp, dp, ucp, vp]
+        L.phx_evolve_device.argtypes = [vp, C.c_int, C.c_double, dp, dp, dp, dp, dp, ucp, vp]
         L.phx_evolve_host.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp, vp, C.POINTER(C.c_double), vp]
         L.phx_debug_flux.argtypes = [vp, C.c_int, dp, vp]
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
@@ -219,6 +220,16 @@ def rk2_step_cfl(mesh, cfl, d_dt, cons0, cons, prim, mask, stream=None):
     _check(lib().phx_rk2_step_cfl(mesh.handle, float(cfl), _dev(d_dt, torch.float64, 1, "d_dt"), _dev(cons0, torch.float64, n, "cons0"),
                                   _dev(cons, torch.float64, n, "cons"), _dev(prim, torch.float64, n, "prim"),
                                   _dev(mask, torch.uint8, mesh.mask_elems, "mask"), _stream(stream)))
+
+
+def evolve_device(mesh, nsteps, cfl, d_dt, cons0, cons, prim, mask, d_t=None, stream=None):
+    """`nsteps` RK2 steps with dt kept on the device (= nsteps x rk2_step_cfl, replayed from a CUDA graph for nsteps >= 2).
+    d_t: optional 1-element CUDA fp64 tensor accumulating the elapsed time."""
+    n = mesh.field_elems
+    _check(lib().phx_evolve_device(mesh.handle, int(nsteps), float(cfl), _dev(d_dt, torch.float64, 1, "d_dt"),
+                                   _dev(d_t, torch.float64, 1, "d_t") if d_t is not None else None,
+                                   _dev(cons0, torch.float64, n, "cons0"), _dev(cons, torch.float64, n, "cons"),
+                                   _dev(prim, torch.float64, n, "prim"), _dev(mask, torch.uint8, mesh.mask_elems, "mask"), _stream(stream)))
 
 
 def _host(t, dtype, numel, name, nullable=False):
