@@ -380,6 +380,31 @@ def smooth_scalar(p, seed, lo=0.1, hi=0.5):
     return lo + (hi - lo) * X
 
 
+def smooth_periodic_prims(p, device="cpu"):
+    """Analytic smooth periodic primitives for a single-block periodic Minkowski mesh, written with torch on `device`
+    straight into the allocated layout [1, 8, nz+2g, ny+2g, nx+2g] (the functions are periodic, so the ghost zones are
+    consistent by construction).  For meshes too large to build on the host (the > 2^31-element indexing test)."""
+    import math
+    import torch
+    assert p["nbx"] == p["nby"] == p["nbz"] == 1
+    gx, gy, gz = ghosts(p)
+    co = []
+    for d, (n, g) in enumerate(((p["nx"], gx), (p["ny"], gy), (p["nz"], gz))):
+        i = torch.arange(-g, n + g, dtype=torch.float64, device=device)
+        co.append(2.0 * math.pi * (i + 0.5) / n)                # phase 2 pi (x - xmin)/L at the cell centres
+    x = co[0][None, None, :]; y = co[1][None, :, None]; z = co[2][:, None, None]
+    q = torch.empty((1, NV, len(co[2]), len(co[1]), len(co[0])), dtype=torch.float64, device=device)
+    q[0, 0] = 1.0 + 0.2 * torch.sin(x) * torch.cos(y) + 0.1 * torch.sin(2.0 * z)
+    q[0, 1] = 0.2 * torch.sin(y) * torch.cos(z)
+    q[0, 2] = 0.15 * torch.sin(z + 0.3) * torch.cos(x)
+    q[0, 3] = -0.1 * torch.sin(x + y)
+    q[0, 4] = 1.5 + 0.3 * torch.cos(x) * torch.sin(z) + 0.1 * torch.cos(2.0 * y)
+    q[0, 5] = 0.5 + 0.1 * torch.sin(y) + 0.0 * x + 0.0 * z
+    q[0, 6] = 0.3 + 0.1 * torch.sin(z) + 0.0 * x + 0.0 * y
+    q[0, 7] = 0.2 + 0.1 * torch.sin(x) + 0.0 * y + 0.0 * z
+    return q
+
+
 def reblock(p, prim_blocks, nb):
     """Same global data on a different block decomposition (for the block-invariance pin)."""
     tot = (p["nbx"] * p["nx"], p["nby"] * p["ny"], p["nbz"] * p["nz"])

@@ -185,3 +185,62 @@ def test_next3_packed_blocks_scalar_radial_floors_sampled():
     w = wl.with_scalar(w, wl.smooth_scalar(w["params"], wl.SEED0 + 9))
     n, s = 256, CORE + 2 * HALO
     run_full(w, [(112, 112, 112), (0, 0, 0), (n - s, n - s, n - s), (100, 120, 90), (176, 16, 208)], check_conservation=False)
+
+
+def test_largest_mesh_indexing_beyond_2_to_31_elements():
+    """Maximum size: one 1024 x 1024 x 256 block (2.25e9 doubles per field, 18 GB; the whole state with flux scratch is
+    108 GB of the 180 GB) so that element offsets exceed 2^31 in every kernel.  Inputs are analytic smooth periodic fields
+    written on the device (workloads.smooth_periodic_prims); one RK2 step with a fixed dt; the oracle reproduces sampled
+    16^3 cores from (16+2*HALO)^3 sub-boxes cut out of the initial state, including cells of the last variables at high k
+    whose offsets lie beyond 2^31."""
+    import torch
+    from paper_2410_09146_b200 import phx
+    free, total = torch.cuda.mem_get_info()
+    if free < 125e9:
+        pytest.skip("needs ~110 GB of free device memory")
+    n = (1024, 1024, 256)
+    p = wl.default_params(nx=n[0], ny=n[1], nz=n[2], ng=4, recon=wl.RECON_PLM_MC, riemann=wl.RIEMANN_HLL, gamma_ad=5.0 / 3.0,
+                          xmax=(4.0, 4.0, 1.0))
+    prim = wl.smooth_periodic_prims(p, "cuda")
+    assert prim.numel() > 2 ** 31
+    mesh = phx.init_mesh(p)
+    cons = torch.empty_like(prim); cons0 = torch.empty_like(prim)
+    mask = torch.zeros((1,) + tuple(prim.shape[2:]), dtype=torch.uint8, device="cuda")
+    d_dt = torch.zeros(1, dtype=torch.float64, device="cuda")
+    s = CORE + 2 * HALO
+    g = p["ng"]
+    origins = [(0, 0, 0), (n[0] - s + 5, n[1] - s + 3, n[2] - s + 7), (500, 1000, 236), (1010, 17, 200), (333, 777, 120)]
+    subs = []
+    for o in origins:       # sub-boxes of the initial state (periodic wrap), pulled to the host before the step
+        idx = [(torch.arange(o[d], o[d] + s, device="cuda") % n[d]) + g for d in range(3)]
+        q = prim[0][:, idx[2]][:, :, idx[1]][:, :, :, idx[0]].cpu().numpy()
+        dx = [(p["xmax"][d] - p["xmin"][d]) / n[d] for d in range(3)]
+        ps = dict(p, nx=s, ny=s, nz=s, xmin=tuple(p["xmin"][d] + o[d] * dx[d] for d in range(3)),
+                  xmax=tuple(p["xmin"][d] + (o[d] + s) * dx[d] for d in range(3)))
+        subs.append((ps, wl.finish(ps, np.ascontiguousarray(q))))
+    dt = 0.2 * (p["xmax"][0] - p["xmin"][0]) / n[0]          # all signal speeds are below 1
+    phx.prim_to_cons(mesh, prim, cons)
+    d_dt.fill_(dt)
+    phx.rk2_step(mesh, d_dt, cons0, cons, prim, mask)
+    torch.cuda.synchronize()
+    assert not bool(mask.bitwise_and(16 | 32).any())
+    scale = cons[0].abs().amax(dim=(1, 2, 3)).cpu().numpy()
+    for o, (ps, sprim) in zip(origins, subs):
+        orc.reset_c2p_margin()
+        r = orc.Run(ps, sprim)
+        r.step(dt)
+        assert orc.last_c2p_margin() > 1e-9
+        oc = wl.from_blocks(ps, r.cons)[:, HALO:HALO + CORE, HALO:HALO + CORE, HALO:HALO + CORE]
+        om = wl.from_blocks(ps, r.mask[:, None])[0][HALO:HALO + CORE, HALO:HALO + CORE, HALO:HALO + CORE]
+        idx = [(torch.arange(o[d] + HALO, o[d] + HALO + CORE, device="cuda") % n[d]) + g for d in range(3)]
+        got = cons[0][:, idx[2]][:, :, idx[1]][:, :, :, idx[0]].cpu().numpy()
+        gm = mask[0][idx[2]][:, idx[1]][:, :, idx[0]].cpu().numpy()
+        err = np.abs(got - oc).reshape(8, -1).max(axis=1) / scale
+        assert err.max() <= TOL_1STEP, f"sub-box at {o}: errors {err}"
+        assert np.array_equal(gm, om)
+    # the last cell of the last variable sits beyond 2^31 elements and was written
+    flat_last = ((7 * prim.shape[2] + (n[2] + g - 1)) * prim.shape[3] + (n[1] + g - 1)) * prim.shape[4] + (n[0] + g - 1)
+    assert flat_last > 2 ** 31
+    mesh.free()
+    del prim, cons, cons0, mask
+    torch.cuda.empty_cache()
