@@ -137,8 +137,13 @@ int phx_evolve_device(phx_mesh* mesh, int nsteps, double cfl, double* d_dt, doub
 int phx_evolve_host(phx_mesh* mesh, const double* h_prim_in, int nsteps, double cfl, double* h_prim_out,
                     double* h_cons_out, unsigned char* h_mask_out, double* h_t, void* stream);
 
-/* Raw Riemann face fluxes F~^d (before flux-CT) of the last stage, for debugging and tests: copies the mesh-owned
- * scratch of direction d (0,1,2) into d_out (DEVICE, phx_field_elems doubles, layout of one 8-variable field,
+/* The sweeps store only what the update needs from other cells: the magnetic components of F~^d (flux-CT); the divergence
+ * of D, S_j, tau (and the passive scalar) is accumulated on the fly.  phx_debug_enable_flux(mesh, 1) makes every later
+ * stage store all components of F~^d as well, for phx_debug_flux. */
+int phx_debug_enable_flux(phx_mesh* mesh, int on);
+
+/* Raw Riemann face fluxes F~^d (before flux-CT) of the last stage (after phx_debug_enable_flux(mesh, 1)), for debugging and
+ * tests: copies the mesh-owned scratch of direction d (0,1,2) into d_out (DEVICE, phx_field_elems doubles, layout of one 8-variable field,
  * the face (i-1/2) stored at cell i), asynchronously on `stream`.  PHX_EINVAL for an inactive direction. */
 int phx_debug_flux(const phx_mesh* mesh, int d, double* d_out, void* stream);
 

@@ -19,13 +19,13 @@ using namespace phx;
 
 // ================================================================================================ kernels
 // launch shapes (tuned on B200 with ncu, profiles/): threads per block and minimum resident blocks per SM; the x sweep is
-// bound to 6 blocks/SM for WENO5-Z-AOAH and to 5 for Kerr-Schild with PLM (96 registers, no spills: 0.90 -> 0.83 ms on
-// 512 blocks of 32^3), WENO5-Z keeps its 128 registers (more blocks per SM measured slower there)
+// bound to 6 blocks/SM for WENO5-Z-AOAH, to 5 for PLM (96 registers, no spills: 0.90 -> 0.83 ms on 512 Kerr-Schild blocks
+// of 32^3) and to 4 for WENO5-Z / MP5 (121 registers; more blocks per SM measured slower there)
 #ifndef PHX_XS_BLOCK
 #define PHX_XS_BLOCK 128
 #endif
 #ifndef PHX_XS_MINB
-#define PHX_XS_MINB 1
+#define PHX_XS_MINB 4
 #endif
 #ifndef PHX_MS_BLOCK
 #define PHX_MS_BLOCK 64
@@ -81,16 +81,28 @@ __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G
 
 // ---- x sweep ------------------------------------------------------------------------------------
 // position p = row*rowlen + ii, cell i = g0-1+ii of row (b, k0+kk, j0+jj); thread t>=1 with ii>=1 owns face (i-1/2).
+// The flux divergence of the non-magnetic components is accumulated by the sweeps themselves into racc (layout
+// [block][NH][k][j][i], NH = 5 + NS: D, S_j, tau and the passive scalar): R <- R - (F_{+1/2} - F_{-1/2})/dx, the first active
+// direction starting from zero.  Only the magnetic components of the fluxes, which flux-CT needs at neighbouring cells, are
+// stored (all components when `store_all` is set: phx_debug_flux).  The sweeps are fp64-bound with HBM to spare, the update
+// is HBM-bound: this moves 80 bytes per zone of flux reads out of the update.
+template <int NS>
+__device__ __forceinline__ int hydro_var(int h) { return h < 5 ? h : XS; }   // h-th accumulated component -> variable index
+
 template <int METRIC, int RECON, int NS>
-__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : (METRIC == 1 && RECON <= 2 ? 5 : PHX_XS_MINB))) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
-                                                      int nplane, int rowlen, int j0, int k0) {
-  // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii)
+__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : (RECON <= 2 ? 5 : PHX_XS_MINB))) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+                                                      double* __restrict__ racc, int store_all, int nplane, int rowlen, int j0, int k0) {
+  // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii);
+  // consecutive thread blocks overlap by two positions: thread 0 only supplies the left state of thread 1's face, the last
+  // thread only the upper face of the cell before it
   constexpr int HW = ReconTraits<RECON>::HW;
-  __shared__ double sh[NV + NS][XS_BLOCK];
-  const int t = threadIdx.x;
-  const int p = blockIdx.x * (XS_BLOCK - 1) + t;
-  const bool valid = p < nplane;
   constexpr int NQ = NV + NS;
+  constexpr int NH = 5 + NS;
+  __shared__ double sh[NQ][XS_BLOCK];
+  __shared__ double shF[NH][XS_BLOCK];
+  const int t = threadIdx.x;
+  const int p = blockIdx.x * (XS_BLOCK - 2) + t;
+  const bool valid = p < nplane;
   double qm[NQ], qp[NQ];
   long long base = 0;
   int ii = 0, i = 0, j = 0, k = 0;
@@ -123,22 +135,41 @@ __global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : (METRIC == 1 && RE
     for (int v = 0; v < NQ; ++v) sh[v][t] = qp[v];
   }
   __syncthreads();
-  if (!valid || t == 0 || ii == 0) return;
-  double qL[NQ];
-#pragma unroll
-  for (int v = 0; v < NQ; ++v) qL[v] = sh[v][t - 1];
-  int cb[3];
-  block_coords(m, b, cb);
-  Geo<METRIC> G;
-  G.at(m, xface(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
+  const bool face = valid && t > 0 && ii > 0;          // this thread owns the face (i-1/2)
   double F[NQ];
-  face_flux<METRIC, 0, NS>(m, G, qL, qm, F);
+  if (face) {
+    double qL[NQ];
 #pragma unroll
-  for (int v = 0; v < NQ; ++v) flux[base + v * m.ncell] = F[v];
+    for (int v = 0; v < NQ; ++v) qL[v] = sh[v][t - 1];
+    int cb[3];
+    block_coords(m, b, cb);
+    Geo<METRIC> G;
+    G.at(m, xface(m, 0, cb[0], i), xcen(m, 1, cb[1], j), xcen(m, 2, cb[2], k));
+    face_flux<METRIC, 0, NS>(m, G, qL, qm, F);
+#pragma unroll
+    for (int h = 0; h < NH; ++h) shF[h][t] = F[hydro_var<NS>(h)];
+  }
+  __syncthreads();
+  if (!face || t > XS_BLOCK - 2) return;               // the last thread's face belongs to the next block's thread 1
+  if (store_all) {
+#pragma unroll
+    for (int v = 0; v < NQ; ++v) flux[base + v * m.ncell] = F[v];
+  } else {
+    flux[base + BY * m.ncell] = F[BY];
+    flux[base + BZ * m.ncell] = F[BZ];
+  }
+  // cell (i, j, k): interior along x (ii <= n) and in the transverse directions
+  if (ii <= m.n[0] && j >= m.g[1] && j < m.g[1] + m.n[1] && k >= m.g[2] && k < m.g[2] + m.n[2]) {
+    const long long rb = (long long)b * NH * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
+#pragma unroll
+    for (int h = 0; h < NH; ++h) racc[rb + h * m.ncell] = 0.0 - (shF[h][t + 1] - F[hydro_var<NS>(h)]) * m.rdx[0];
+  }
 }
 
 // ---- y / z sweep ---------------------------------------------------------------------------------
-// Lanes along x (coalesced); every thread marches along the sweep direction over one segment of faces.  The (2*HW+1)-row
+// Lanes along x (coalesced); every thread marches along the sweep direction over one segment of cells c0..c1: it computes
+// the faces c0..c1+1 (the last one again belongs to the next segment, which stores it), keeps the previous face's flux
+// and accumulates the divergence of the non-magnetic components of the cells in between into racc.  The (2*HW+1)-row
 // stencil window of its column lives in shared memory as a ring of rows that cp.async fills one row ahead of the
 // arithmetic (each primitive is read from HBM once per segment, no register window, no long-scoreboard stall); a thread
 // reads only its own column of the ring, so no block barrier is needed, only cp.async.wait_group.
@@ -153,11 +184,14 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 template <int METRIC, int RECON, int D, int NS>
 __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+                                                                       double* __restrict__ racc, int store_all, int first,
                                                                        int ntr, int n0, int lo0, int lo1, int L) {
   constexpr int HW = ReconTraits<RECON>::HW;
   constexpr int NW = 2 * HW + 1;   // stencil rows
   constexpr int NR = NW + 1;       // ring: the stencil plus one row in flight
   constexpr int NQ = NV + NS;
+  constexpr int NH = 5 + NS;
+  constexpr int O = (D == 1) ? 2 : 1;   // the other transverse direction
   __shared__ double win[NR][NQ][MS_BLOCK];
   const int tid = threadIdx.x;
   const int p = blockIdx.x * MS_BLOCK + tid;
@@ -169,10 +203,14 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
   const int o = lo1 + t1;             // the other transverse index (k for D=1, j for D=2)
   const long long sd = (D == 1) ? m.sj : m.sk;
   const long long so = (D == 1) ? m.sk : m.sj;
-  const int f0 = m.g[D] + seg * L;
-  const int f1 = min(f0 + L - 1, m.g[D] + m.n[D]);
-  if (f0 > f1) return;
+  const int clast = m.g[D] + m.n[D] - 1;          // last interior cell along D
+  const int f0 = m.g[D] + seg * L;                // first cell (and first face) of this segment
+  const int c1 = min(f0 + L - 1, clast);          // last cell
+  if (f0 > c1) return;
+  const int f1 = c1 + 1;                          // last face computed here
   const long long col = (long long)b * m.nvar * m.ncell + (long long)o * so + i;
+  const long long rcol = (long long)b * NH * m.ncell + (long long)o * so + i;
+  const bool inner = i >= m.g[0] && i < m.g[0] + m.n[0] && o >= m.g[O] && o < m.g[O] + m.n[O];   // interior column
   int cb[3];
   block_coords(m, b, cb);
   const double xx = xcen(m, 0, cb[0], i);
@@ -190,10 +228,27 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
   }
   int s0 = 0;                                     // ring slot of row c-HW
   int snew = NW;                                  // ring slot the next prefetched row goes to
+  // rst: divergence accumulated so far in the cell below the current face, fetched at the top of the iteration; fst: the
+  // previous face's flux.  Kerr-Schild keeps both in shared memory (own column only, cp.async) to spare registers
+  // (0.86 -> 0.78 ms on 512 blocks of 32^3); the flat metrics keep them in registers (PLM 0.55 vs 0.57 ms at 256^3).
+  constexpr bool RSM = (METRIC == 1);
+  __shared__ double rst[RSM ? NH : 1][MS_BLOCK];
+  __shared__ double fst[RSM ? NH : 1][MS_BLOCK];
+  double Rreg[NH], Freg[NH];
+#pragma unroll
+  for (int h = 0; h < NH; ++h) { Rreg[h] = 0.0; Freg[h] = 0.0; }
   double qpPrev[NQ];
 #pragma unroll
   for (int v = 0; v < NQ; ++v) qpPrev[v] = 0.0;
   for (int c = f0 - 1; c <= f1; ++c) {
+    const bool cell = inner && c >= f0 + 1;
+    if (cell && !first) {
+#pragma unroll
+      for (int h = 0; h < NH; ++h) {
+        if constexpr (RSM) cp_async8(&rst[h][tid], racc + rcol + h * m.ncell + (long long)(c - 1) * sd);
+        else Rreg[h] = racc[rcol + h * m.ncell + (long long)(c - 1) * sd];
+      }
+    }
     if (c + HW + 1 <= rlast) {
 #pragma unroll
       for (int v = 0; v < NQ; ++v) cp_async8(&win[snew][v][tid], src + v * m.ncell);
@@ -229,8 +284,29 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
       if (D == 1) G.at(m, xx, xf, xo); else G.at(m, xx, xo, xf);
       double F[NQ];
       face_flux<METRIC, D, NS>(m, G, qpPrev, qm, F);
+      if (c <= c1 || c == clast + 1) {            // the face c1+1 is stored by the next segment unless it is the last face
+        if (store_all) {
 #pragma unroll
-      for (int v = 0; v < NQ; ++v) flux[col + v * m.ncell + (long long)c * sd] = F[v];
+          for (int v = 0; v < NQ; ++v) flux[col + v * m.ncell + (long long)c * sd] = F[v];
+        } else {
+          flux[col + BX * m.ncell + (long long)c * sd] = F[BX];
+          flux[col + (D == 1 ? BZ : BY) * m.ncell + (long long)c * sd] = F[D == 1 ? BZ : BY];
+        }
+      }
+      if (cell) {
+        if constexpr (RSM) cp_async_wait<0>();    // rst (and the row in flight) have landed long ago
+#pragma unroll
+        for (int h = 0; h < NH; ++h) {
+          const double Rold = first ? 0.0 : (RSM ? rst[h][tid] : Rreg[h]);
+          const double Fp = RSM ? fst[h][tid] : Freg[h];
+          racc[rcol + h * m.ncell + (long long)(c - 1) * sd] = Rold - (F[hydro_var<NS>(h)] - Fp) * m.rdx[D];
+        }
+      }
+#pragma unroll
+      for (int h = 0; h < NH; ++h) {
+        if constexpr (RSM) fst[h][tid] = F[hydro_var<NS>(h)];
+        else Freg[h] = F[hydro_var<NS>(h)];
+      }
     }
 #pragma unroll
     for (int v = 0; v < NQ; ++v) qpPrev[v] = qp[v];
@@ -241,7 +317,7 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
 }
 
 // ---- update: flux-CT + divergence + sources + RK combine + con2prim + floors ----------------------
-struct FluxPtrs { const double* f[3]; };
+struct FluxPtrs { const double* f[3]; const double* racc; };
 
 // contribution of the edge-EMF pair (A, C) (third direction E) to d/dt of B~^C and B~^A, reading C5.3
 template <int A, int C, bool EXC>
@@ -318,13 +394,17 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
   double R[NQ];
 #pragma unroll
   for (int v = 0; v < NQ; ++v) R[v] = 0.0;
+  // D, S_j, tau (and the passive scalar, which has no source: S = 0 in Eq.14): the divergence the sweeps accumulated
+  if (m.act[0] || m.act[1] || m.act[2]) {
+    constexpr int NH = 5 + NS;
+    const double* A = fl.racc + (long long)b * NH * m.ncell + c;
+#pragma unroll
+    for (int h = 0; h < NH; ++h) R[hydro_var<NS>(h)] = A[h * m.ncell];
+  }
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     if (!m.act[d]) continue;
     const double* F = fl.f[d] + vb + c;
-#pragma unroll
-    for (int v = 0; v <= CTAU; ++v) R[v] -= (F[v * m.ncell + str[d]] - F[v * m.ncell]) * m.rdx[d];
-    if constexpr (NS == 1) R[XS] -= (F[XS * m.ncell + str[d]] - F[XS * m.ncell]) * m.rdx[d];   // no source: S = 0 in Eq.14
     // magnetic components that flux-CT does not replace (inactive partner direction, or CT switched off)
 #pragma unroll
     for (int cc = 0; cc < 3; ++cc) {
@@ -651,6 +731,8 @@ struct phx_mesh {
   MeshDev m;
   phx_params par;
   double* flux[3];
+  double* racc;               // divergence of the non-magnetic flux components accumulated by the sweeps: [block][5+nscalar][cells]
+  int store_all_fluxes;       // phx_debug_enable_flux: the sweeps also store the non-magnetic flux components
   unsigned char* xfl;
   double* partial;
   int npartial;
@@ -770,6 +852,13 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
     e = cudaMemsetAsync(M->flux[d], 0, fbytes, st);
     if (e != cudaSuccess) { phx_free_mesh(M); return cuda_fail(e, "cudaMemsetAsync"); }
   }
+  {
+    const size_t rbytes = (size_t)M->nall * (5 + p->nscalar) * sizeof(double);
+    cudaError_t e = cudaMalloc((void**)&M->racc, rbytes);
+    if (e != cudaSuccess) { phx_free_mesh(M); return (e == cudaErrorMemoryAllocation) ? fail(PHX_ENOMEM, "phx_init_mesh: out of device memory (divergence scratch)") : cuda_fail(e, "cudaMalloc"); }
+    e = cudaMemsetAsync(M->racc, 0, rbytes, st);
+    if (e != cudaSuccess) { phx_free_mesh(M); return cuda_fail(e, "cudaMemsetAsync"); }
+  }
   M->npartial = 148 * 8;
   if (cudaMalloc((void**)&M->partial, sizeof(double) * M->npartial) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
   if (cudaMalloc((void**)&M->smax, sizeof(unsigned long long) * PHX_NSLOT) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
@@ -788,6 +877,7 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
 extern "C" int phx_free_mesh(phx_mesh* M) {
   if (!M) return PHX_OK;
   for (int d = 0; d < 3; ++d) if (M->flux[d]) cudaFree(M->flux[d]);
+  if (M->racc) cudaFree(M->racc);
   if (M->xfl) cudaFree(M->xfl);
   if (M->partial) cudaFree(M->partial);
   if (M->smax) cudaFree(M->smax);
@@ -806,6 +896,12 @@ extern "C" int phx_free_mesh(phx_mesh* M) {
 extern "C" size_t phx_field_elems(const phx_mesh* M) { return M ? (size_t)M->nall * M->m.nvar : 0; }
 extern "C" size_t phx_mask_elems(const phx_mesh* M) { return M ? (size_t)M->nall : 0; }
 extern "C" unsigned long long phx_launch_count(const phx_mesh* M) { return M ? M->launches : 0; }
+extern "C" int phx_debug_enable_flux(phx_mesh* M, int on) {
+  if (!M) return fail(PHX_EINVAL, "phx_debug_enable_flux: null mesh");
+  M->store_all_fluxes = on ? 1 : 0;
+  return PHX_OK;
+}
+
 extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* stream) {
   if (!M || d < 0 || d > 2 || !M->flux[d] || !aligned16(d_out)) return fail(PHX_EINVAL, "phx_debug_flux: null argument or inactive direction");
   CUDA_TRY(cudaMemcpyAsync(d_out, M->flux[d], (size_t)M->nall * M->m.nvar * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream), "cudaMemcpyAsync");
@@ -883,15 +979,16 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
   if (m.act[0]) {
     const int rowlen = m.n[0] + 2;
     const int nplane = cnt[1] * rowlen;
-    dim3 grid((nplane + (XS_BLOCK - 2)) / (XS_BLOCK - 1), cnt[2], m.nblk);
+    dim3 grid((nplane - 1 + (XS_BLOCK - 3)) / (XS_BLOCK - 2), cnt[2], m.nblk);   // every position >= 1 is some block's thread 1..XS_BLOCK-2
     ProfScope ps(M, PHX_K_SWEEP_X, st);
-    k_sweep_x<METRIC, RECON, NS><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], nplane, rowlen, lo[1], lo[2]);
+    k_sweep_x<METRIC, RECON, NS><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], M->racc, M->store_all_fluxes, nplane, rowlen, lo[1], lo[2]);
     M->launches++;
   }
   // Segments of at most 33 faces along the sweep direction; a small mesh gets more, shorter segments (at least 4 faces)
   // until the launch has about four waves of thread blocks, so that the marching sweeps do not starve for parallelism
   // (64^3: 2 segments = 0.9 blocks per SM -> 17 segments).  The fluxes do not depend on the segmentation.
-  auto segments = [&](int nfaces, int ntr) {
+  auto segments = [&](int ncells, int ntr) {
+    const int nfaces = ncells;
     int nseg = (nfaces + 32) / 33;
     const long long per_seg = (long long)((ntr + MS_BLOCK - 1) / MS_BLOCK) * m.nblk;
     const long long want = 148LL * PHX_MS_MINB * 4;
@@ -901,23 +998,23 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     return nseg < 1 ? 1 : nseg;
   };
   if (m.act[1]) {
-    const int nfaces = m.n[1] + 1;
+    const int ncells = m.n[1];
     const int ntr = cnt[0] * cnt[2];
-    const int nseg = segments(nfaces, ntr);
-    const int L = (nfaces + nseg - 1) / nseg;
+    const int nseg = segments(ncells, ntr);
+    const int L = (ncells + nseg - 1) / nseg;
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Y, st);
-    k_sweep_march<METRIC, RECON, 1, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], ntr, cnt[0], lo[0], lo[2], L);
+    k_sweep_march<METRIC, RECON, 1, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], M->racc, M->store_all_fluxes, m.act[0] ? 0 : 1, ntr, cnt[0], lo[0], lo[2], L);
     M->launches++;
   }
   if (m.act[2]) {
-    const int nfaces = m.n[2] + 1;
+    const int ncells = m.n[2];
     const int ntr = cnt[0] * cnt[1];
-    const int nseg = segments(nfaces, ntr);
-    const int L = (nfaces + nseg - 1) / nseg;
+    const int nseg = segments(ncells, ntr);
+    const int L = (ncells + nseg - 1) / nseg;
     dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Z, st);
-    k_sweep_march<METRIC, RECON, 2, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], ntr, cnt[0], lo[0], lo[1], L);
+    k_sweep_march<METRIC, RECON, 2, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], M->racc, M->store_all_fluxes, (m.act[0] || m.act[1]) ? 0 : 1, ntr, cnt[0], lo[0], lo[1], L);
     M->launches++;
   }
 }
@@ -941,6 +1038,7 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
   { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
   FluxPtrs fl;
   for (int d = 0; d < 3; ++d) fl.f[d] = M->flux[d];
+  fl.racc = M->racc;
   const dim3 nb((M->m.n[0] * M->m.n[1] + UP_BLOCK - 1) / UP_BLOCK, M->m.n[2], M->m.nblk);
   {
   ProfScope ps(M, PHX_K_UPDATE, st);

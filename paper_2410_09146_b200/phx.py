@@ -25,7 +25,7 @@ EXPORTS = (
     "phx_init_mesh", "phx_free_mesh", "phx_field_elems", "phx_mask_elems", "phx_prim_to_cons",
     "phx_cons_to_prim", "phx_fill_ghosts", "phx_rk_stage", "phx_cfl_dt", "phx_rk2_step",
     "phx_evolve_host", "phx_debug_flux", "phx_launch_count", "phx_last_error",
-    "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl", "phx_evolve_device",
+    "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl", "phx_evolve_device", "phx_debug_enable_flux",
 )
 
 
@@ -95,6 +95,7 @@ def lib():
         L.phx_evolve_device.argtypes = [vp, C.c_int, C.c_double, dp, dp, dp, dp, dp, ucp, vp]
         L.phx_evolve_host.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp, vp, C.POINTER(C.c_double), vp]
         L.phx_debug_flux.argtypes = [vp, C.c_int, dp, vp]
+        L.phx_debug_enable_flux.argtypes = [vp, C.c_int]
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
         L.phx_profile_enable.argtypes = [vp, C.c_int]
         L.phx_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
@@ -138,6 +139,10 @@ class Mesh:
 
     def launch_count(self) -> int:
         return int(lib().phx_launch_count(self.handle))
+
+    def debug_enable_flux(self, on=True):
+        """Make the sweeps store every component of the raw Riemann fluxes (needed before debug_flux)."""
+        _check(lib().phx_debug_enable_flux(self.handle, 1 if on else 0))
 
     def debug_flux(self, d, shape, stream=None):
         """Copy of the mesh-owned raw Riemann flux of direction d as a CUDA tensor of `shape`."""

@@ -191,6 +191,7 @@ def test_raw_riemann_fluxes_match_oracle_without_ct(name):
     F = orc.stage_fluxes(p, w["prim"])
     # a zero-dt stage leaves the state alone and the raw fluxes in the mesh-owned scratch
     g2 = GpuRun(p, w["prim"])
+    g2.mesh.debug_enable_flux(True)        # the sweeps otherwise store the magnetic components only
     phx.rk_stage(g2.mesh, 1.0, 0.0, 0.0, g2.cons, g2.cons, g2.prim, g2.mask)
     gx, gy, gz = wl.ghosts(p)
     nx, ny, nz = p["nx"], p["ny"], p["nz"]
