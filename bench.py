@@ -35,27 +35,28 @@ METRIC = "grmhd_zone_cycles_per_sec"
 UNIT = "zone-cycles/s"
 
 # Algorithmic traffic and arithmetic per interior zone and launch.
-# Bytes: what the kernel's definition must move.  update = 3 x 7 flux components read (the d-th magnetic component of F~^d
-# is identically zero and not needed) + U~0 read + U~1 read (stage 2 only: 32 B averaged over both stages) + 5 primitives
-# read (sources / con2prim guess) + U~ and P written + mask.
+# Bytes: what the kernel's definition must move.  The sweeps read P (64 B), write the two magnetic flux components flux-CT
+# needs (16 B) and accumulate the divergence of the five non-magnetic components (x: 40 B written; y, z: 40 B read + 40 B
+# written).  update = that divergence (40 B) + 3 x 2 magnetic flux components (48 B) + U~0 read + U~1 read (stage 2 only:
+# 32 B averaged over both stages) + 5 primitives read (sources / con2prim guess) + U~ and P written + mask.
 ALGO_BYTES_PER_ZONE = {
-    "sweep_x": 128.0, "sweep_y": 128.0, "sweep_z": 128.0,       # read P (64 B), write F~ (64 B)
-    "update": 168.0 + 64.0 + 32.0 + 40.0 + 64.0 + 64.0 + 1.0,
+    "sweep_x": 64.0 + 16.0 + 40.0, "sweep_y": 64.0 + 16.0 + 80.0, "sweep_z": 64.0 + 16.0 + 80.0,
+    "update": 40.0 + 48.0 + 64.0 + 32.0 + 40.0 + 64.0 + 64.0 + 1.0,
     "fill_ghosts": 0.0, "cfl": 64.0, "prim_to_cons": 128.0, "c2p": 129.0, "copy": 128.0,
 }
 # fp64 flop per interior zone and launch for the WENO5-Z + HLL Minkowski path: dadd + dmul + 2*dfma thread-instructions of
 # the committed kernels counted by ncu (profiles/r01_ncu_summary.md; con2prim iterations are data dependent, the figure
 # is the one measured on this workload).  achieved = these flops / measured time, i.e. useful fp64 work only.
-# update: average of the first stage (670) and the second stage, which also evaluates the signal speeds for the fused CFL
-# reduction (798); the "cfl" class is the one-block final kernel of that reduction
-ALGO_FLOP_PER_ZONE = {"sweep_x": 1071.0, "sweep_y": 1085.0, "sweep_z": 1085.0, "update": 734.0, "cfl": 0.0}
+# update: average of the first stage (631) and the second stage, which also evaluates the signal speeds for the fused CFL
+# reduction (760); the "cfl" class is the one-block final kernel of that reduction
+ALGO_FLOP_PER_ZONE = {"sweep_x": 1106.0, "sweep_y": 1141.0, "sweep_z": 1141.0, "update": 695.0, "cfl": 0.0}
 # fp64 peak from unit counts and clocks: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz; a DFMA loop measured
 # 33.9 TFLOP/s on this pool's B200 (16.94 T DFMA/s)
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 FP64_MEASURED_DFMA_TFLOPS = 33.9
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (bytes)
-NCU_TRAFFIC = {256: {"update": 7.725e9, "sweep_x": 2.206e9, "sweep_y": 2.304e9, "sweep_z": 2.301e9, "cfl": 0.0,
-                     "fill_ghosts": 0.256e9}}
+NCU_TRAFFIC = {256: {"update": 6.126e9, "sweep_x": 2.040e9, "sweep_y": 2.797e9, "sweep_z": 2.796e9, "cfl": 0.0,
+                     "fill_ghosts": 0.255e9}}
 
 
 def parse_args():
