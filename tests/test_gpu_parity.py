@@ -311,6 +311,30 @@ def test_two_dimensional_run_matches_oracle():
 
 
 # ----------------------------------------------------------------------------- error behaviour of the C ABI
+@pytest.mark.parametrize("shape", [(1, 20, 28), (1, 1, 40), (1, 36, 1), (24, 1, 20)])
+def test_meshes_with_inactive_leading_dimensions_match_oracle(shape):
+    """Inactive x (and y): the first active sweep starts the divergence accumulator, flux-CT acts only on the active pair,
+    1-D runs along y or z go through the marching sweep alone.  shape = (nx, ny, nz)."""
+    nx, ny, nz = shape
+    p = wl.default_params(nx=nx, ny=ny, nz=nz, ng=3, recon=wl.RECON_WENO5Z, riemann=wl.RIEMANN_HLL)
+    rng = np.random.default_rng(wl.SEED0 + 40 + nx + 3 * ny + 7 * nz)
+    q = np.zeros((8, nz, ny, nx))
+    q[0] = 1.0 + 0.2 * rng.uniform(-1, 1, q[0].shape)
+    q[1:4] = 0.2 * rng.uniform(-1, 1, q[1:4].shape)
+    q[4] = 1.0 + 0.2 * rng.uniform(-1, 1, q[0].shape)
+    q[5:8] = 0.3 * rng.uniform(-1, 1, q[1:4].shape)
+    for d, n in enumerate((nx, ny, nz)):
+        if sum(m > 1 for m in (nx, ny, nz)) == 1 and n > 1:
+            q[5 + d] = 0.4                       # 1-D: the normal field must be uniform (div B = 0)
+    prim = wl.finish(p, q)
+    o, g = run_both(p, prim, nsteps=3)
+    compare(p, o, g, TOL_1STEP * 10)
+    # scalar-carrying variant of the same mesh
+    w = wl.with_scalar(dict(name="inactive", params=p, prim=prim, cfl=0.4), 0.2 + 0.1 * rng.uniform(0, 1, (nz, ny, nx)))
+    o, g = run_both(w["params"], w["prim"], nsteps=2)
+    compare(w["params"], o, g, TOL_1STEP * 10)
+
+
 def test_c_abi_rejects_bad_arguments():
     torch, phx = _gpu()
     p = wl.default_params(nx=16, ny=16, nz=16, ng=2, recon=wl.RECON_WENO5Z)
