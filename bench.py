@@ -9,8 +9,8 @@ box (WENO5-Z, HLL, flux-CT, RK2, Minkowski, Gamma=5/3) that north_star's rooflin
 seeded synthetic fields from paper_2410_09146_b200/workloads.py (recipe in DESIGN.md section 4).
 
 value     : interior zones x K / device time (CUDA events, max over ranks), state resident in HBM.
-e2e       : same metric through phx_evolve_host (HOST buffers: H2D of the primitives and D2H of primitives,
-            conserved variables and mask inside the timed region, one call per step).
+e2e       : same metric through phx_evolve_host (HOST buffers: H2D of the primitives and D2H of the new primitives
+            and the mask inside the timed region, one call per step).
 roofline  : dominant kernel class, per-launch time from CUDA events recorded by the library on the launching
             stream inside the timed region (phx_profile_*), algorithmic bytes / flops per zone from DESIGN.md 6.
 cpu_baseline : the oracle (oracle/, as it stands) on a bounded sample of the same workload on the host cores.
@@ -309,20 +309,21 @@ def run_ours(args):
         del cons0
         torch.cuda.empty_cache()
         hin = h_prim.pin_memory()
-        hp = torch.empty_like(hin).pin_memory(); hc = torch.empty_like(hin).pin_memory()
+        hp = torch.empty_like(hin).pin_memory()
         hm = torch.empty(mask.shape, dtype=torch.uint8).pin_memory()
         ke = max(1, min(K, 3))
-        phx.evolve_host(mesh, hin, 1, w["cfl"], hp, hc, hm)        # warm-up (allocates the workspace)
+        # the step's result is the new state: the primitives (they determine U~) and the con2prim / floor mask
+        phx.evolve_host(mesh, hin, 1, w["cfl"], hp, None, hm)      # warm-up (allocates the workspace)
         barrier()
         e0.record()
         for _ in range(ke):
-            phx.evolve_host(mesh, hin, 1, w["cfl"], hp, hc, hm)
+            phx.evolve_host(mesh, hin, 1, w["cfl"], hp, None, hm)
         e1.record()
         barrier()
         _, e2e_value = aggregate(e0.elapsed_time(e1), zones, ke, world, "cuda")
         e2e = {"value": e2e_value, "unit": UNIT,
-               "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": 2 * field_bytes + hm.numel() + 16,
-               "steps": ke, "call": "phx_evolve_host(nsteps=1) per step, pinned host buffers"}
+               "h2d_bytes_per_step": field_bytes, "d2h_bytes_per_step": field_bytes + hm.numel() + 16,
+               "steps": ke, "call": "phx_evolve_host(nsteps=1) per step, pinned host buffers: primitives in; primitives and mask out"}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
