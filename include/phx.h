@@ -69,7 +69,8 @@ typedef struct {
   double floor_alpha_rho, floor_alpha_eps; /* exponents alpha of the density and specific-energy floors (paper: 2.0) */
 } phx_params;
 
-/* Build a mesh object: validates the parameters, allocates flux scratch (3 x one field),
+/* Build a mesh object: validates the parameters, allocates flux scratch (3 x one field) and the divergence accumulator
+ * (5 + nscalar variables of one field: the sweeps add -(F_{+1/2} - F_{-1/2})/dx of D, S_j, tau and the scalar to it),
  * the excision flag array and reduction scratch, and runs the geometry-flag kernel on `stream`.
  * Errors: PHX_EINVAL (bad sizes, ng too small for recon, inactive dimension split over blocks),
  * PHX_ENOMEM, PHX_ECUDA.  The mesh is freed with phx_free_mesh. */
@@ -143,7 +144,7 @@ int phx_evolve_host(phx_mesh* mesh, const double* h_prim_in, int nsteps, double 
 int phx_debug_enable_flux(phx_mesh* mesh, int on);
 
 /* Raw Riemann face fluxes F~^d (before flux-CT) of the last stage (after phx_debug_enable_flux(mesh, 1)), for debugging and
- * tests: copies the mesh-owned scratch of direction d (0,1,2) into d_out (DEVICE, phx_field_elems doubles, layout of one 8-variable field,
+ * tests: copies the mesh-owned scratch of direction d (0,1,2) into d_out (DEVICE, phx_field_elems doubles, layout of one field,
  * the face (i-1/2) stored at cell i), asynchronously on `stream`.  PHX_EINVAL for an inactive direction. */
 int phx_debug_flux(const phx_mesh* mesh, int d, double* d_out, void* stream);
 
