@@ -428,6 +428,39 @@ def test_boosted_linear_waves_converge_on_the_papers_grid_range(kind):
     assert min(slopes) > 1.7 and slopes[-1] > 1.9 and math.log2(errs[0] / errs[-1]) / 5 > 1.85, (errs, slopes)
 
 
+def test_sedov_blast_at_the_papers_size_follows_the_self_similar_solution():
+    """The paper's scaling workload (3-D Sedov-Taylor blast, 128^3) on the CUDA path against the Newtonian
+    self-similar solution R(t) = 1.15167 (E t^2 / rho)^(1/5) (Gamma = 5/3; the oracle is pinned to it at 32^3, P14):
+    density peak on an axis and on the diagonal within one zone, octant symmetry, energy conserved while the shock is
+    inside the domain, no floor or failure anywhere."""
+    import math
+    n = 128
+    w = wl.sedov_blast(n)
+    p = w["params"]
+    g = GpuRun(p, w["prim"])
+    tau0 = interior(p, g.get()[0])[4].sum(dtype=np.longdouble)
+    t, t_end, nsteps = 0.0, 30.0, 0
+    while t < t_end:
+        dt = min(g.dt(0.4), t_end - t)
+        g.step(dt)
+        t += dt
+        nsteps += 1
+    cons, prim, mask1, mask = g.get()
+    assert not mask.any() and not mask1.any()
+    rho = interior(p, prim)[0]
+    h = 2.0 / n
+    R = 1.15167 * (1e-5 * t_end ** 2) ** 0.2
+    c = n // 2
+    r_axis = (np.argmax(rho[c, c, c:]) + 0.5) * h
+    r_diag = (np.argmax([rho[c + i, c + i, c + i] for i in range(n // 2)]) + 0.5) * h * math.sqrt(3.0)
+    print("Sedov 128^3:", nsteps, "steps, R =", R, "axis", r_axis, "diagonal", r_diag, "rho_max", rho.max())
+    assert abs(r_axis - R) <= 1.5 * h and abs(r_diag - R) <= 1.5 * h * math.sqrt(3.0), (r_axis, r_diag, R)
+    assert np.abs(rho - rho[::-1, :, :]).max() < 1e-9 and np.abs(rho - rho.transpose(2, 1, 0)).max() < 1e-9
+    assert rho.max() > 2.0 and rho[c, c, c] < 0.1 and abs(rho[c, c, -1] - 1.0) < 1e-12
+    tau1 = interior(p, cons)[4].sum(dtype=np.longdouble)
+    assert abs(float((tau1 - tau0) / tau0)) < 1e-11
+
+
 def test_bondi_inflow_matches_oracle_and_stays_stationary():
     """Pin P13's exact stationary solution (Bondi inflow, Kerr-Schild a = 0) through the CUDA path: parity with the oracle
     over 12 steps and the same stationarity away from the outflow faces."""
