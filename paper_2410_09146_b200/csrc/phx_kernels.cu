@@ -1,13 +1,16 @@
 // phx_kernels.cu — sm_100a kernels and the C ABI of include/phx.h.
 //
 // Kernels per Runge-Kutta stage (all launched on the caller's stream, no host synchronisation):
-//   k_sweep_x      fused reconstruct + Riemann flux along x: one thread per cell, upper-face states exchanged through
-//                  shared memory, flat tiling over (row, i) so that warps stay full for any row length
-//   k_sweep_march  fused reconstruct + Riemann flux along y or z: lanes along x (coalesced), each thread marches along
-//                  the sweep direction with a register window of 2*HW+1 rows, so every primitive is loaded once
-//   k_update       flux-CT + flux divergence + geometric sources + RK combine + con2prim + floors, one thread per cell
-//   k_fill_ghosts  periodic / outflow / block-to-block ghost copies in one gather pass
-// and k_cfl_partial / k_cfl_final (warp-shuffle min reduction), k_prim_to_cons, k_c2p, k_excision_flags.
+//   k_sweep_x      fused reconstruct + Riemann flux along x: one thread per cell, upper-face states and face fluxes exchanged
+//                  through shared memory, flat tiling over (row, i) so that warps stay full for any row length
+//   k_sweep_march  fused reconstruct + Riemann flux along y or z: lanes along x (coalesced), each thread marches along the
+//                  sweep direction; the 2*HW+1 stencil rows of its column sit in a shared-memory ring that cp.async fills
+//                  one row ahead, so every primitive is read from HBM once
+//                  (all three sweeps store the magnetic flux components and accumulate the divergence of the others)
+//   k_update       flux-CT + accumulated divergence + geometric sources + RK combine + con2prim + floors, one thread per cell
+//   k_fill_ghosts  periodic / outflow / block-to-block ghost copies in one gather pass over the ghost cells
+// and k_cfl_partial / k_cfl_final (warp-shuffle min reduction), k_cfl_final_slots (fused into stage 2), k_prim_to_cons,
+// k_c2p, k_excision_flags; phx_evolve_device replays one captured step as a CUDA graph.
 #include "phx_device.cuh"
 #include "../../include/phx.h"
 
