@@ -23,7 +23,9 @@
 //
 // P16 passive scalar (Eq.14): constant X stays constant, sum of sqrt(gamma) D X conserved, smooth profile advected at
 // second order, bounds; P17 floor forms of PAPER.md:288 against the closed-form Kerr-Schild radius on the axis, in the
-// equatorial plane and for a = 0.
+// equatorial plane and for a = 0.  P18 (tests/test_oracle_pins_positivity.py): the positivity fallback of the fifth-order
+// reconstructions in block_fluxes (which cell, which direction, all variables, threshold <= the floors at the cell centre,
+// never for piecewise-linear schemes) on hand-worked stencils.
 //
 // Layout of every field: [block][var][k][j][i], i fastest; var order of primitives
 // P=(rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3) (Eq.13) and conserved, stored densitised,
