@@ -105,7 +105,8 @@ int phx_rk_stage(phx_mesh* mesh, double g0, double g1, double beta_dt, const dou
 
 /* dt = cfl * min over interior, non-excised cells of 1 / sum_d max(|lambda+^d|, |lambda-^d|)/dx_d.
  * d_dt (device, required) receives the result; if h_dt is non-NULL the value is also copied to the host
- * and the stream is synchronised. */
+ * and the stream is synchronised.  A cell whose speeds are not finite (NaN primitives) makes the result NaN rather than
+ * being skipped; a mesh without any evolving cell gives +inf.  The fused reductions of phx_rk2_step_cfl behave the same. */
 int phx_cfl_dt(const phx_mesh* mesh, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream);
 
 /* One full RK2 step with the time step read from the device scalar d_dt (no host round trip); the result equals two
@@ -160,6 +161,13 @@ enum { PHX_K_SWEEP_X = 0, PHX_K_SWEEP_Y = 1, PHX_K_SWEEP_Z = 2, PHX_K_UPDATE = 3
        PHX_K_PRIM_TO_CONS = 6, PHX_K_C2P = 7, PHX_K_COPY = 8, PHX_K_COUNT = 9 };
 int phx_profile_enable(phx_mesh* mesh, int max_records);
 int phx_profile_read(phx_mesh* mesh, double* h_ms, unsigned long long* h_count);
+
+/* Peak of the fp64 pipe, measured: a loop of independent fused multiply-adds (8 chains per thread, 64 warps per SM) on every
+ * SM for at least `min_seconds` (0 < min_seconds <= 10) after a calibration launch, timed with CUDA events on `stream`.
+ * *h_dfma_per_s (HOST, required) receives DFMA thread-instructions per second (x 2 = flop/s); *h_ms (HOST, nullable) the
+ * duration of the timed launch; *h_nsm (HOST, nullable) the SM count of the current device.  Synchronises `stream`.
+ * The denominator of bench.py's ALU roofline (R64 is to be measured, not assumed). */
+int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, double* h_ms, int* h_nsm, void* stream);
 
 const char* phx_last_error(void);
 

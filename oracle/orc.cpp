@@ -927,6 +927,7 @@ int orc_cfl_dt(const orc_params* p, const double* prim, double cfl, double* dt) 
   Grid G(*p);
   double best = std::numeric_limits<double>::infinity();
   for (int b = 0; b < G.nblk; ++b)
+#pragma omp parallel for collapse(2) schedule(static) reduction(min : best) if ((long)G.n[1] * G.n[2] > 1)
     for (int k = G.g[2]; k < G.g[2] + G.n[2]; ++k)
       for (int j = G.g[1]; j < G.g[1] + G.n[1]; ++j)
         for (int i = G.g[0]; i < G.g[0] + G.n[0]; ++i) {

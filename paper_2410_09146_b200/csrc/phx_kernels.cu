@@ -322,6 +322,15 @@ __global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m
 // ---- update: flux-CT + divergence + sources + RK combine + con2prim + floors ----------------------
 struct FluxPtrs { const double* f[3]; const double* racc; };
 
+// A cell whose sum_d max|lambda^d|/dx_d is NaN (non-finite primitives) must not be dropped by fmax: it enters the reduction
+// as +inf, and the final kernels turn an infinite maximum into dt = NaN, which no later step can hide.  A mesh without any
+// evolving cell (maximum 0) gets dt = +inf: nothing constrains the step.
+__device__ __forceinline__ double cfl_guard(double s) { return (s >= 0.0) ? s : __longlong_as_double(0x7ff0000000000000LL); }
+__device__ __forceinline__ double cfl_dt_of(double cfl, double vmax) {
+  return isinf(vmax) ? __longlong_as_double(0x7ff8000000000000LL) : cfl * (1.0 / vmax);
+}
+
+
 // contribution of the edge-EMF pair (A, C) (third direction E) to d/dt of B~^C and B~^A, reading C5.3
 template <int A, int C, bool EXC>
 __device__ __forceinline__ void ct_pair(const MeshDev& m, const FluxPtrs& fl, const unsigned char* __restrict__ xfl, long long vb,
@@ -470,7 +479,7 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
     double sum = 0.0;
 #pragma unroll
     for (int d = 0; d < 3; ++d) if (m.act[d]) sum += lam[d] * m.rdx[d];
-    return sum;
+    return cfl_guard(sum);
   }
   return 0.0;
 }
@@ -514,7 +523,7 @@ __global__ void __launch_bounds__(256) k_cfl_final_slots(unsigned long long* __r
     double v = sh[0];
 #pragma unroll
     for (int w = 1; w < 8; ++w) v = fmax(v, sh[w]);
-    *dt = cfl * (1.0 / v);
+    *dt = cfl_dt_of(cfl, v);
   }
 }
 
@@ -673,7 +682,7 @@ __global__ void __launch_bounds__(256) k_cfl_partial(MeshDev m, const unsigned c
     double s = 0.0;
 #pragma unroll
     for (int d = 0; d < 3; ++d) if (m.act[d]) s += lam[d] * m.rdx[d];
-    best = fmax(best, s);
+    best = fmax(best, cfl_guard(s));
   }
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, o));
@@ -700,7 +709,7 @@ __global__ void __launch_bounds__(256) k_cfl_final(const double* __restrict__ pa
     double v = (threadIdx.x < 8) ? sh[threadIdx.x] : 0.0;
 #pragma unroll
     for (int o = 4; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    if (threadIdx.x == 0) *dt = cfl * (1.0 / v);
+    if (threadIdx.x == 0) *dt = cfl_dt_of(cfl, v);
   }
 }
 
@@ -740,16 +749,18 @@ struct phx_mesh {
   double* partial;
   int npartial;
   unsigned long long* smax;   // PHX_NSLOT accumulators of the fused CFL reduction (zero between steps)
-  unsigned long long launches;
+  int nsm;                    // SMs of the device the mesh lives on (launch sizing)
+  // bookkeeping that calls on a const mesh update (launch counter, event records): not part of the mesh's logical state
+  mutable unsigned long long launches;
   long long nall, ninterior;
   // workspace of the host-buffer path (phx_evolve_host), allocated on first use
   double* ws_field[3];
   unsigned char* ws_mask;
   double* ws_scal;   // [0] dt, [1] t
   // per-kernel-class CUDA-event timing (phx_profile_enable / phx_profile_read)
-  cudaEvent_t* ev;   // 2 events per recorded launch
-  int* evcls;
-  int evcap, evn;
+  mutable cudaEvent_t* ev;   // 2 events per recorded launch
+  mutable int* evcls;
+  mutable int evcap, evn;
   // CUDA graph of one RK2 step (phx_evolve_device): captured once per argument set on a mesh-owned stream and replayed
   cudaStream_t gstream;
   cudaEvent_t gev_in, gev_out;
@@ -760,8 +771,8 @@ struct phx_mesh {
 
 // RAII pair of events around one launch (or one group of launches) of class `cls`, recorded on the launching stream
 struct ProfScope {
-  phx_mesh* M; cudaStream_t st; int slot;
-  ProfScope(phx_mesh* M_, int cls, cudaStream_t st_) : M(M_), st(st_), slot(-1) {
+  const phx_mesh* M; cudaStream_t st; int slot;
+  ProfScope(const phx_mesh* M_, int cls, cudaStream_t st_) : M(M_), st(st_), slot(-1) {
     if (M->ev && M->evn < M->evcap) { slot = M->evn++; M->evcls[slot] = cls; cudaEventRecord(M->ev[2 * slot], st); }
   }
   ~ProfScope() { if (slot >= 0) cudaEventRecord(M->ev[2 * slot + 1], st); }
@@ -862,7 +873,14 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
     e = cudaMemsetAsync(M->racc, 0, rbytes, st);
     if (e != cudaSuccess) { phx_free_mesh(M); return cuda_fail(e, "cudaMemsetAsync"); }
   }
-  M->npartial = 148 * 8;
+  {
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) {
+      cudaGetLastError(); phx_free_mesh(M); return fail(PHX_ECUDA, "phx_init_mesh: cannot query the SM count of the device");
+    }
+    M->nsm = nsm;
+  }
+  M->npartial = M->nsm * 8;
   if (cudaMalloc((void**)&M->partial, sizeof(double) * M->npartial) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
   if (cudaMalloc((void**)&M->smax, sizeof(unsigned long long) * PHX_NSLOT) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ENOMEM, "phx_init_mesh: out of device memory"); }
   if (cudaMemsetAsync(M->smax, 0, sizeof(unsigned long long) * PHX_NSLOT, st) != cudaSuccess) { phx_free_mesh(M); return fail(PHX_ECUDA, "phx_init_mesh: cudaMemsetAsync failed"); }
@@ -901,7 +919,9 @@ extern "C" size_t phx_mask_elems(const phx_mesh* M) { return M ? (size_t)M->nall
 extern "C" unsigned long long phx_launch_count(const phx_mesh* M) { return M ? M->launches : 0; }
 extern "C" int phx_debug_enable_flux(phx_mesh* M, int on) {
   if (!M) return fail(PHX_EINVAL, "phx_debug_enable_flux: null mesh");
-  M->store_all_fluxes = on ? 1 : 0;
+  const int v = on ? 1 : 0;
+  if (v != M->store_all_fluxes && M->gexec) { cudaGraphExecDestroy(M->gexec); M->gexec = nullptr; }   // the flag is baked into the captured launches
+  M->store_all_fluxes = v;
   return PHX_OK;
 }
 
@@ -918,8 +938,7 @@ extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* str
     else { CALL(2); }                               \
   } while (0)
 
-extern "C" int phx_prim_to_cons(const phx_mesh* Mc, const double* d_prim, double* d_cons, void* stream) {
-  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+extern "C" int phx_prim_to_cons(const phx_mesh* M, const double* d_prim, double* d_cons, void* stream) {
   if (!M || !aligned16(d_prim) || !aligned16(d_cons)) return fail(PHX_EINVAL, "phx_prim_to_cons: null or misaligned argument");
   cudaStream_t st = (cudaStream_t)stream;
   const unsigned nb = (unsigned)((M->nall + 255) / 256);
@@ -933,8 +952,7 @@ extern "C" int phx_prim_to_cons(const phx_mesh* Mc, const double* d_prim, double
   return PHX_OK;
 }
 
-extern "C" int phx_fill_ghosts(const phx_mesh* Mc, double* d_prim, void* stream) {
-  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+extern "C" int phx_fill_ghosts(const phx_mesh* M, double* d_prim, void* stream) {
   if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
   if (M->nall == M->ninterior) return PHX_OK;
   { ProfScope ps(M, PHX_K_FILL_GHOSTS, (cudaStream_t)stream);
@@ -946,8 +964,7 @@ extern "C" int phx_fill_ghosts(const phx_mesh* Mc, double* d_prim, void* stream)
   return PHX_OK;
 }
 
-extern "C" int phx_cons_to_prim(const phx_mesh* Mc, double* d_cons, double* d_prim, unsigned char* d_mask, void* stream) {
-  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+extern "C" int phx_cons_to_prim(const phx_mesh* M, double* d_cons, double* d_prim, unsigned char* d_mask, void* stream) {
   if (!M || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask) return fail(PHX_EINVAL, "phx_cons_to_prim: null or misaligned argument");
   cudaStream_t st = (cudaStream_t)stream;
   const unsigned nb = (unsigned)((M->ninterior + UP_BLOCK - 1) / UP_BLOCK);
@@ -994,7 +1011,7 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
     const int nfaces = ncells;
     int nseg = (nfaces + 32) / 33;
     const long long per_seg = (long long)((ntr + MS_BLOCK - 1) / MS_BLOCK) * m.nblk;
-    const long long want = 148LL * PHX_MS_MINB * 4;
+    const long long want = (long long)M->nsm * PHX_MS_MINB * 4;
     const int need = (int)((want + per_seg - 1) / per_seg);
     const int cap = (nfaces + 3) / 4;
     if (need > nseg) nseg = need < cap ? need : cap;
@@ -1096,8 +1113,7 @@ extern "C" int phx_rk2_step_cfl(phx_mesh* M, double cfl, double* d_dt, double* d
   return PHX_OK;
 }
 
-extern "C" int phx_cfl_dt(const phx_mesh* Mc, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream) {
-  phx_mesh* M = const_cast<phx_mesh*>(Mc);
+extern "C" int phx_cfl_dt(const phx_mesh* M, const double* d_prim, double cfl, double* d_dt, double* h_dt, void* stream) {
   if (!M || !aligned16(d_prim) || !d_dt || !(cfl > 0.0)) return fail(PHX_EINVAL, "phx_cfl_dt: null or misaligned argument, or cfl <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   long long want = (M->ninterior + 255) / 256;
@@ -1145,6 +1161,58 @@ extern "C" int phx_profile_read(phx_mesh* M, double* h_ms, unsigned long long* h
     h_count[M->evcls[i]]++;
   }
   M->evn = 0;
+  return PHX_OK;
+}
+
+// ---- fp64 pipe peak: a DFMA loop on every SM (bench.py's ALU roofline denominator, measured in the same run) ---------------
+// 8 independent fused multiply-add chains per thread, 64 warps per SM: nothing but the fp64 pipe limits it.
+__global__ void __launch_bounds__(256) k_fp64_peak(double* __restrict__ sink, long long iters, double a, double b) {
+  double x[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) x[k] = 1.0 + 1e-3 * k + 1e-9 * threadIdx.x;
+  for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+#pragma unroll
+      for (int k = 0; k < 8; ++k) x[k] = fma(x[k], a, b);
+    }
+  }
+  double t = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) t += x[k];
+  if (t == 123456.789) sink[0] = t;      // never true: keeps the chains alive
+}
+
+extern "C" int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, double* h_ms, int* h_nsm, void* stream) {
+  if (!(min_seconds > 0.0) || min_seconds > 10.0 || !h_dfma_per_s) return fail(PHX_EINVAL, "phx_debug_fp64_peak: min_seconds in (0, 10] and a result pointer required");
+  cudaStream_t st = (cudaStream_t)stream;
+  int dev = 0, nsm = 0;
+  CUDA_TRY(cudaGetDevice(&dev), "cudaGetDevice");
+  CUDA_TRY(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute");
+  double* sink = nullptr;
+  CUDA_TRY(cudaMalloc((void**)&sink, sizeof(double)), "cudaMalloc");
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  const int nblk = nsm * 8;
+  const double per_iter = (double)nblk * 256.0 * 32.0;          // DFMA thread-instructions per loop iteration
+  long long iters = 1 << 14;
+  float ms = 0.f;
+  cudaError_t e = cudaSuccess;
+  for (int pass = 0; pass < 3 && e == cudaSuccess; ++pass) {    // warm-up / calibration, then the timed launch
+    cudaEventRecord(e0, st);
+    k_fp64_peak<<<nblk, 256, 0, st>>>(sink, iters, 0.999999, 1e-6);
+    cudaEventRecord(e1, st);
+    e = cudaEventSynchronize(e1);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    if (pass == 2 || e != cudaSuccess) break;
+    const double rate = per_iter * (double)iters / (ms * 1e-3);
+    iters = (long long)(min_seconds * rate / per_iter * (pass == 0 ? 0.05 : 1.0)) + 1;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  if (e != cudaSuccess) return cuda_fail(e, "k_fp64_peak");
+  *h_dfma_per_s = per_iter * (double)iters / (ms * 1e-3);
+  if (h_ms) *h_ms = ms;
+  if (h_nsm) *h_nsm = nsm;
   return PHX_OK;
 }
 
@@ -1215,12 +1283,11 @@ extern "C" int phx_evolve_host(phx_mesh* M, const double* h_prim_in, int nsteps,
   if (!M || !h_prim_in || !h_prim_out || nsteps < 0 || !(cfl > 0.0)) return fail(PHX_EINVAL, "phx_evolve_host: null argument, nsteps < 0 or cfl <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   const size_t fbytes = (size_t)M->nall * M->m.nvar * sizeof(double);
-  if (!M->ws_scal) {
-    for (int d = 0; d < 3; ++d)
-      if (cudaMalloc((void**)&M->ws_field[d], fbytes) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
-    if (cudaMalloc((void**)&M->ws_mask, (size_t)M->nall) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
-    if (cudaMalloc((void**)&M->ws_scal, 2 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
-  }
+  // each buffer is allocated once; a failure part-way leaves the ones already there for the next call (freed with the mesh)
+  for (int d = 0; d < 3; ++d)
+    if (!M->ws_field[d] && cudaMalloc((void**)&M->ws_field[d], fbytes) != cudaSuccess) { M->ws_field[d] = nullptr; cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
+  if (!M->ws_mask && cudaMalloc((void**)&M->ws_mask, (size_t)M->nall) != cudaSuccess) { M->ws_mask = nullptr; cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
+  if (!M->ws_scal && cudaMalloc((void**)&M->ws_scal, 2 * sizeof(double)) != cudaSuccess) { M->ws_scal = nullptr; cudaGetLastError(); return fail(PHX_ENOMEM, "phx_evolve_host: out of device memory"); }
   double* prim = M->ws_field[0];
   double* cons = M->ws_field[1];
   double* cons0 = M->ws_field[2];

@@ -26,6 +26,7 @@ EXPORTS = (
     "phx_cons_to_prim", "phx_fill_ghosts", "phx_rk_stage", "phx_cfl_dt", "phx_rk2_step",
     "phx_evolve_host", "phx_debug_flux", "phx_launch_count", "phx_last_error",
     "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl", "phx_evolve_device", "phx_debug_enable_flux",
+    "phx_debug_fp64_peak",
 )
 
 
@@ -99,6 +100,7 @@ def lib():
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
         L.phx_profile_enable.argtypes = [vp, C.c_int]
         L.phx_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
+        L.phx_debug_fp64_peak.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int), vp]
         L.phx_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -255,3 +257,10 @@ def evolve_host(mesh, h_prim_in, nsteps, cfl, h_prim_out, h_cons_out=None, h_mas
                                  _host(h_cons_out, torch.float64, n, "h_cons_out", True),
                                  _host(h_mask_out, torch.uint8, mesh.mask_elems, "h_mask_out", True), C.byref(t), _stream(stream)))
     return t.value
+
+
+def debug_fp64_peak(min_seconds=0.5, stream=None):
+    """Measured peak of the fp64 pipe: (DFMA thread-instructions per second, milliseconds of the timed launch, SM count)."""
+    r, ms, nsm = C.c_double(), C.c_double(), C.c_int()
+    _check(lib().phx_debug_fp64_peak(float(min_seconds), C.byref(r), C.byref(ms), C.byref(nsm), _stream(stream)))
+    return r.value, ms.value, nsm.value

@@ -316,43 +316,114 @@ def sedov_blast(n=128, E=1e-5, r_init=0.1, recon=RECON_PLM_MINMOD):
     return dict(name="next2_sedov_blast", params=p, prim=finish(p, q), cfl=0.4, steps=20)
 
 
+def linear_mode(kind, rho0, P0, gam, Bpar, Bperp, direction=1):
+    """Closed-form linear eigenmode of ideal relativistic MHD about a fluid at rest (the exact solution the linear-wave
+    inputs sample; PAPER.md:430-441 names the four families).  Wave normal n, background field B = Bpar n + Bperp t with t a
+    unit vector orthogonal to n, third direction z = n x t.  Linearising Eq.1-3 about v = 0 with a = rho h, E = a + B^2:
+      drho = rho v_n / lam,  dP = a c_s^2 v_n / lam,  dB_t = (Bperp v_n - Bpar v_t)/lam,  dB_z = -Bpar v_z / lam,
+      [lam^2 (a + Bperp^2) - a c_s^2 - Bperp^2] v_n - Bpar Bperp (lam^2 - 1) v_t = 0,
+      Bpar Bperp (lam^2 - 1) v_n - [lam^2 (a + Bpar^2) - Bpar^2] v_t = 0,       E lam^2 v_z = Bpar^2 v_z,
+    so lam^2 solves  E s^2 - (B^2 + a c_s^2 + c_s^2 Bpar^2) s + c_s^2 Bpar^2 = 0  (fast: larger root, slow: smaller root),
+    lam_Alfven^2 = Bpar^2 / E, and with Bperp = 0 the roots are c_s^2 (sound) and the Alfven speed.
+    Returns the perturbation per unit amplitude (normalised to drho = rho0 for the compressive modes, dv_z = 1 for Alfven)
+    of a wave travelling along direction * n: dict(lam, drho, dP, dvn, dvt, dvz, dBt, dBz)."""
+    a = rho0 + P0 / (gam - 1.0) + P0
+    cs2 = gam * P0 / a
+    B2 = Bpar * Bpar + Bperp * Bperp
+    E = a + B2
+    out = dict(drho=0.0, dP=0.0, dvn=0.0, dvt=0.0, dvz=0.0, dBt=0.0, dBz=0.0)
+    if kind == "alfven":
+        lam = direction * abs(Bpar) / np.sqrt(E)
+        out.update(lam=lam, dvz=1.0, dBz=-Bpar / lam)
+        return out
+    if kind == "sound":
+        if Bperp != 0.0:
+            raise ValueError("a pure sound wave needs the field along the wave normal (or none)")
+        s = cs2
+    else:
+        b = B2 + a * cs2 + cs2 * Bpar * Bpar
+        disc = np.sqrt(b * b - 4.0 * E * cs2 * Bpar * Bpar)
+        if kind == "fast":
+            s = (b + disc) / (2.0 * E)
+        elif kind == "slow":
+            s = 2.0 * cs2 * Bpar * Bpar / (b + disc)      # the smaller root, without cancellation
+        else:
+            raise ValueError(kind)
+    lam = direction * np.sqrt(s)
+    vn = lam                                              # drho = rho0
+    vt = Bpar * Bperp * (s - 1.0) * vn / (s * (a + Bpar * Bpar) - Bpar * Bpar) if Bperp != 0.0 else 0.0
+    out.update(lam=lam, drho=rho0, dP=a * cs2, dvn=vn, dvt=vt, dBt=(Bperp * vn - Bpar * vt) / lam)
+    return out
+
+
+WAVE_KINDS = ("sound", "alfven", "fast", "slow")          # PAPER.md:441
+WAVE_BPAR, WAVE_BPERP = 1.0, 1.5                          # background field of the magnetosonic waves (the paper gives none)
+
+
+def _wave_background(kind):
+    """(Bpar, Bperp) of the background of each family: none for sound, along n for Alfven, oblique for fast / slow."""
+    return {"sound": (0.0, 0.0), "alfven": (1.0, 0.0)}.get(kind, (WAVE_BPAR, WAVE_BPERP))
+
+
+def linear_wave_1d(n=64, kind="sound", A=1e-6, recon=RECON_PLM_MC, riemann=RIEMANN_HLL):
+    """SURVEY.md 8(c) pin P9: 1-D linear wave on the periodic unit interval, Minkowski, Gamma = 5/3, rho = P = 1 at rest,
+    one wavelength, travelling towards +x: the eigenmode of `linear_mode` with n = x, t = y.  Returns the workload plus
+    the period and the variable the L1 norm of Eq.61 is taken of.  No RNG."""
+    gam = 5.0 / 3.0
+    p = default_params(nx=n, ng=2 if recon in (1, 2) else 3, gamma_ad=gam, recon=recon, riemann=riemann)
+    x = cell_centres(p)[0]
+    s = np.sin(2.0 * np.pi * x)
+    Bpar, Bperp = _wave_background(kind)
+    m = linear_mode(kind, 1.0, 1.0, gam, Bpar, Bperp, +1)
+    q = np.zeros((NV, 1, 1, n))
+    q[0, 0, 0] = 1.0 + A * m["drho"] * s
+    q[4, 0, 0] = (1.0 + A * m["dP"] * s) / (gam - 1.0)
+    v = A * np.array([m["dvn"], m["dvt"], m["dvz"]])[:, None] * s[None, :]
+    W = 1.0 / np.sqrt(1.0 - (v * v).sum(0))
+    q[1:4, 0, 0] = W * v
+    q[5, 0, 0] = Bpar
+    q[6, 0, 0] = Bperp + A * m["dBt"] * s
+    q[7, 0, 0] = A * m["dBz"] * s
+    var = 7 if kind == "alfven" else 0
+    return dict(name=f"p9_{kind}_wave", params=p, prim=finish(p, q), cfl=0.4, steps=None, period=1.0 / abs(m["lam"]), var=var,
+                amplitude=A * (abs(m["dBz"]) if kind == "alfven" else 1.0), mode=m)
+
+
 def boosted_linear_wave(n=64, kind="sound", boost=0.617213, A=1e-6, recon=RECON_PLM_MC):
     """the paper's linear-wave set-up: 2-D, Gamma = 5/3, flat metric with
-    coordinate boosts v_x = v_y = 0.617213, periodic unit square.  Background rho = P = 1 at rest in the unboosted frame;
-    a plane wave of amplitude A with phase 2 pi (x + y) travelling against the boost (so that one period of the pattern in
-    the boosted coordinates is short): sound (drho = A rho, dP = A rho h c_s^2, dv = -A c_s n) or Alfven with B_0 = 1 along
-    n = (1,1)/sqrt 2 (dv_z = A, dB_z = +A sqrt(rho h + B_0^2)).  Returns the workload plus the period T of the pattern
-    and the index of the variable the L1 norm of Eq.61 is taken of.  No RNG."""
+    coordinate boosts v_x = v_y = 0.617213, periodic unit square, the four families sound, Alfven, fast and slow magnetosonic
+    (PAPER.md:441).  Background rho = P = 1 at rest in the unboosted frame; a plane wave of amplitude A with phase
+    2 pi (x + y), wave normal n = (1,1)/sqrt 2, travelling against the boost (so that one period of the pattern in the boosted
+    coordinates is short); t = (-1,1)/sqrt 2.  Sound: no field; Alfven: B_0 = 1 along n; fast / slow: B_0 = 1 n + 1.5 t (the
+    paper prints no background).  The perturbation is the closed-form eigenmode of `linear_mode`.
+    Returns the workload plus the period T of the pattern and the index of the variable the L1 norm of Eq.61 is taken
+    of.  No RNG."""
     gam = 5.0 / 3.0
     p = default_params(metric=MINKOWSKI_BOOSTED, shift=(boost, boost, 0.0), nx=n, ny=n, nz=1, ng=2 if recon in (1, 2) else 3,
                        gamma_ad=gam, recon=recon, riemann=RIEMANN_HLL)
     x, y, _ = cell_centres(p)
     Y, X = np.meshgrid(y, x, indexing="ij")
     s = np.sin(2.0 * np.pi * (X + Y))[None]           # [1, Ny, Nx]
-    rho0, P0, B0 = 1.0, 1.0, 1.0
-    rhoh = rho0 + P0 / (gam - 1.0) + P0
-    q = np.zeros((NV, 1, n, n))
-    q[0], q[4] = rho0, P0 / (gam - 1.0)
+    Bpar, Bperp = _wave_background(kind)
+    m = linear_mode(kind, 1.0, 1.0, gam, Bpar, Bperp, -1)
     r2 = np.sqrt(0.5)
-    if kind == "sound":
-        cs = np.sqrt(gam * P0 / rhoh)
-        q[0] += A * rho0 * s
-        q[4] += A * rhoh * cs * cs * s / (gam - 1.0)
-        v = -A * cs * s
-        W = 1.0 / np.sqrt(1.0 - v * v)
-        q[1], q[2] = W * v * r2, W * v * r2
-        lam, var = cs, 0
-    elif kind == "alfven":
-        q[5], q[6] = B0 * r2, B0 * r2
-        lam = B0 / np.sqrt(rhoh + B0 * B0)
-        v = A * s
-        q[3] = v / np.sqrt(1.0 - v * v)
-        q[7] = A * np.sqrt(rhoh + B0 * B0) * s
-        var = 7
-    else:
-        raise ValueError(kind)
-    T = 1.0 / (np.sqrt(2.0) * lam + 2.0 * boost)
-    return dict(name=f"next4_boosted_{kind}_wave", params=p, prim=finish(p, q), cfl=0.4, steps=None, period=T, var=var, amplitude=A)
+    nx_, ny_, tx_, ty_ = r2, r2, -r2, r2
+    q = np.zeros((NV, 1, n, n))
+    q[0] = 1.0 + A * m["drho"] * s
+    q[4] = (1.0 + A * m["dP"] * s) / (gam - 1.0)
+    vn, vt, vz = A * m["dvn"] * s, A * m["dvt"] * s, A * m["dvz"] * s
+    W = 1.0 / np.sqrt(1.0 - (vn * vn + vt * vt + vz * vz))
+    q[1] = W * (vn * nx_ + vt * tx_)
+    q[2] = W * (vn * ny_ + vt * ty_)
+    q[3] = W * vz
+    Bt = Bperp + A * m["dBt"] * s
+    q[5] = Bpar * nx_ + Bt * tx_
+    q[6] = Bpar * ny_ + Bt * ty_
+    q[7] = A * m["dBz"] * s
+    var = 7 if kind == "alfven" else 0
+    T = 1.0 / (np.sqrt(2.0) * abs(m["lam"]) + 2.0 * boost)
+    return dict(name=f"next4_boosted_{kind}_wave", params=p, prim=finish(p, q), cfl=0.4, steps=None, period=T, var=var,
+                amplitude=A * (abs(m["dBz"]) if kind == "alfven" else 1.0), mode=m)
 
 
 def with_scalar(w, X, scalar_min=0.0, scalar_max=1.0):

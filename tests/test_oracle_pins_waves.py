@@ -1,0 +1,156 @@
+"""Pins P9 / P15 of the CPU oracle for the paper's four linear-wave families: "sound, Alfven, fast, and slow magnetosonic
+waves" (section 4.1.1, Figs 1-4), 1-D unboosted and 2-D on the flat metric with
+coordinate boosts v_x = v_y = 0.617213.
+
+The eigenmodes the inputs sample come from the closed form in workloads.linear_mode.  They are pinned here against
+something else: the flux Jacobian (dU/dP)^-1 dF/dP of Eq.2-3, with U(P) and F(P) written out in this file in
+numpy for flat space and differentiated numerically - no oracle routine and no workloads routine enters that matrix.
+The oracle's own point-wise U and F are then checked against the same numpy restatement, and the full scheme is run
+over one period: the wave must come back to where it started with an L1 error (Eq.61) that falls at
+"roughly at least the expected second order".  All of these run without a GPU.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import orc
+from paper_2410_09146_b200 import workloads as wl
+
+GAM = 5.0 / 3.0
+ETA = np.diag([-1.0, 1.0, 1.0, 1.0])
+
+
+# ----------------------------------------------------------------------------- Eq.2-3 in flat space, numpy only
+def cons_flux_flat(q, gam=GAM):
+    """U (Eq.2) and F^x (Eq.3) of the primitives q = (rho, W v^i, rho eps, B^i) for alpha = 1, beta = 0, gamma_ij = delta_ij."""
+    rho, ut, u, B = q[0], q[1:4], q[4], q[5:8]
+    W = math.sqrt(1.0 + ut @ ut)
+    v = ut / W
+    P = (gam - 1.0) * u
+    b0 = W * (B @ v)                                   # Eq.10 (alpha = 1)
+    bi = B / W + b0 * v                                # Eq.11
+    b2 = (B @ B) / W ** 2 + (B @ v) ** 2               # Eq.12
+    w = rho + u + P + b2
+    D = rho * W
+    S = w * W * W * v - b0 * bi
+    tau = w * W * W - (P + 0.5 * b2) - b0 * b0 - D
+    U = np.concatenate([[D], S, [tau], B])
+    F = np.empty(8)
+    F[0] = D * v[0]
+    F[1:4] = S * v[0] - bi * B[0] / W
+    F[1] += P + 0.5 * b2
+    F[4] = tau * v[0] + (P + 0.5 * b2) * v[0] - b0 * B[0] / W
+    F[5:8] = B * v[0] - B[0] * v
+    return U, F
+
+
+def flux_jacobian(q0):
+    """A = (dU/dP)^-1 dF/dP over the 7 variables (rho, u~x, u~y, u~z, u, By, Bz) (B^x is fixed in 1-D), central differences."""
+    idx = [0, 1, 2, 3, 4, 6, 7]
+    dU = np.empty((7, 7)); dF = np.empty((7, 7))
+    for c, k in enumerate(idx):
+        h = 1e-6
+        qp = q0.copy(); qm = q0.copy()
+        qp[k] += h; qm[k] -= h
+        Up, Fp = cons_flux_flat(qp); Um, Fm = cons_flux_flat(qm)
+        dU[:, c] = (Up - Um)[idx] / (2 * h)
+        dF[:, c] = (Fp - Fm)[idx] / (2 * h)
+    return np.linalg.solve(dU, dF)
+
+
+def background(kind):
+    Bpar, Bperp = wl._wave_background(kind)
+    return np.array([1.0, 0.0, 0.0, 0.0, 1.0 / (GAM - 1.0), Bpar, Bperp, 0.0])
+
+
+def mode_vector(m):
+    """The eigenmode of workloads.linear_mode as a perturbation of (rho, u~x, u~y, u~z, u, By, Bz) (u~ = v at linear order)."""
+    return np.array([m["drho"], m["dvn"], m["dvt"], m["dvz"], m["dP"] / (GAM - 1.0), m["dBt"], m["dBz"]])
+
+
+def test_oracle_point_cons_and_flux_equal_the_numpy_restatement_of_eq2_eq3():
+    rng = np.random.default_rng(7)
+    for _ in range(50):
+        q = np.concatenate([[10 ** rng.uniform(-2, 1)], rng.uniform(-1.5, 1.5, 3), [10 ** rng.uniform(-2, 1)], rng.uniform(-1, 1, 3)])
+        U, F = cons_flux_flat(q)
+        scale = np.abs(U).max() + np.abs(F).max()
+        assert np.abs(orc.point_cons(ETA, GAM, q) - U).max() < 1e-14 * scale
+        assert np.abs(orc.point_flux(ETA, GAM, q, 0) - np.where(np.arange(8) == 5, 0.0, F)).max() < 1e-14 * scale
+
+
+@pytest.mark.parametrize("kind", wl.WAVE_KINDS)
+@pytest.mark.parametrize("direction", [1, -1])
+def test_linear_modes_are_eigenvectors_of_the_numerical_flux_jacobian(kind, direction):
+    q0 = background(kind)
+    A = flux_jacobian(q0)
+    m = wl.linear_mode(kind, 1.0, 1.0, GAM, q0[5], q0[6], direction)
+    r = mode_vector(m)
+    res = np.abs(A @ r - m["lam"] * r).max() / np.abs(r).max()
+    assert res < 2e-9, (kind, res)
+    # all seven characteristic speeds are real and are the ones the closed forms give: 0, +-Alfven, +-fast, +-slow
+    lam = np.sort(np.linalg.eigvals(A).real)
+    assert np.abs(np.linalg.eigvals(A).imag).max() < 1e-7
+    a = 1.0 + 1.0 / (GAM - 1.0) + 1.0
+    Bpar, Bperp = q0[5], q0[6]
+    if Bpar == 0.0 and Bperp == 0.0:
+        want = [-math.sqrt(GAM / a), 0, 0, 0, 0, 0, math.sqrt(GAM / a)]
+    else:
+        la = abs(wl.linear_mode("alfven", 1.0, 1.0, GAM, Bpar, Bperp)["lam"])
+        if Bperp == 0.0:
+            lf, ls = sorted([math.sqrt(GAM / a), la])[::-1]
+        else:
+            lf = abs(wl.linear_mode("fast", 1.0, 1.0, GAM, Bpar, Bperp)["lam"])
+            ls = abs(wl.linear_mode("slow", 1.0, 1.0, GAM, Bpar, Bperp)["lam"])
+        want = [-lf, -la, -ls, 0, ls, la, lf]
+    assert np.abs(lam - np.sort(want)).max() < 2e-7, (lam, want)   # a defective pair of equal speeds splits by sqrt(eps)
+    assert abs(abs(m["lam"]) - {"sound": math.sqrt(GAM / a)}.get(kind, abs(m["lam"]))) < 1e-15
+
+
+def test_magnetosonic_speeds_of_the_oblique_background_bracket_the_alfven_speed():
+    """Textbook ordering slow <= Alfven <= fast < 1, and the numbers of this background (rho = P = 1, B = 1 n + 1.5 t)."""
+    f = wl.linear_mode("fast", 1.0, 1.0, GAM, wl.WAVE_BPAR, wl.WAVE_BPERP)["lam"]
+    s = wl.linear_mode("slow", 1.0, 1.0, GAM, wl.WAVE_BPAR, wl.WAVE_BPERP)["lam"]
+    al = wl.linear_mode("alfven", 1.0, 1.0, GAM, wl.WAVE_BPAR, wl.WAVE_BPERP)["lam"]
+    assert 0 < s < al < f < 1
+    # the oracle's signal-speed bound (reading C4, upper-bound magnetosonic speed) must not be below the true fast speed
+    lm, lp = orc.point_speeds(ETA, GAM, background("fast"), 0)
+    assert lp >= f and lm <= -f
+
+
+# ----------------------------------------------------------------------------- P9: 1-D, unboosted
+def _wave_error(w):
+    p = w["params"]
+    r = orc.Run(p, w["prim"])
+    T = w["period"]
+    while r.t < T * (1 - 1e-12):
+        r.step(min(r.dt(0.4), T - r.t))
+    a = wl.from_blocks(p, r.prim)[w["var"]]
+    b = wl.from_blocks(p, w["prim"])[w["var"]]
+    return np.abs(a - b).sum() / a.size / w["amplitude"]     # L1 norm of Eq.61 in units of the amplitude
+
+
+@pytest.mark.parametrize("kind", ["fast", "slow"])
+def test_p9_magnetosonic_waves_converge_at_second_order(kind):
+    errs = [_wave_error(wl.linear_wave_1d(n, kind)) for n in (64, 128, 256)]
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    print(kind, errs, slopes)
+    assert errs[0] < 0.08                     # the wave came back where it started
+    assert slopes[0] > 1.7 and slopes[1] > 1.85, (errs, slopes)
+
+
+@pytest.mark.parametrize("kind", ["sound", "alfven"])
+def test_p9_closed_form_inputs_reproduce_the_sound_and_alfven_waves(kind):
+    """The same pin as test_p9_linear_waves_converge_at_second_order, through the shared input recipe."""
+    errs = [_wave_error(wl.linear_wave_1d(n, kind)) for n in (64, 128)]
+    assert errs[0] < 0.05 and math.log2(errs[0] / errs[1]) > 1.8, errs
+
+
+# ----------------------------------------------------------------------------- P15: 2-D, boosted
+@pytest.mark.parametrize("kind", ["fast", "slow"])
+def test_p15_boosted_magnetosonic_waves_converge_at_second_order(kind):
+    errs = [_wave_error(wl.boosted_linear_wave(n, kind)) for n in (32, 64)]
+    slope = math.log2(errs[0] / errs[1])
+    print(kind, errs, slope)
+    assert errs[0] < 0.2, errs
+    assert slope > 1.7, (errs, slope)
