@@ -24,7 +24,7 @@
 // P16 passive scalar (Eq.14): constant X stays constant, sum of sqrt(gamma) D X conserved, smooth profile advected at
 // second order, bounds; P17 floor forms of PAPER.md:288 against the closed-form Kerr-Schild radius on the axis, in the
 // equatorial plane and for a = 0.  P18 (tests/test_oracle_pins_positivity.py): the positivity fallback of the fifth-order
-// reconstructions in block_fluxes (which cell, which direction, all variables, threshold <= the floors at the cell centre,
+// reconstructions in block_fluxes (which cell, which direction, all variables, threshold just below the floors at the cell centre,
 // never for piecewise-linear schemes) on hand-worked stencils.
 //
 // Layout of every field: [block][var][k][j][i], i fastest; var order of primitives
@@ -729,11 +729,14 @@ void block_fluxes(const Grid& G, int b, const double* prim, std::vector<double> 
           for (int v = 0; v < nv; ++v) recon_cell(p.recon, P + v * vstr + c, str[d], m[v], pl[v]);
           if (p.recon >= 3) {
             // positivity fallback: piecewise constant in this direction for all variables; the thresholds are the
-            // floors at the centre of the cell
+            // floors at the centre of the cell, lowered by one part in 1e12 (reading C5.1): con2prim holds
+            // whole regions exactly AT the floor, where every reconstruction returns the floor up to rounding; a
+            // threshold at the floor itself would leave the decision there to the last bit of the arithmetic
             const double xc[3] = {G.xc(0, b, i), G.xc(1, b, j), G.xc(2, b, k)};
             double rfl, efl;
             floors_at(p, xc, rfl, efl);
-            if (m[RHO] <= rfl || pl[RHO] <= rfl || m[UU] <= rfl * efl || pl[UU] <= rfl * efl)
+            const double thr_rho = rfl * (1.0 - 1e-12), thr_u = rfl * efl * (1.0 - 1e-12);
+            if (m[RHO] < thr_rho || pl[RHO] < thr_rho || m[UU] < thr_u || pl[UU] < thr_u)
               for (int v = 0; v < nv; ++v) m[v] = pl[v] = P[v * vstr + c];
           }
           for (int v = 0; v < nv; ++v) { qm[v * vstr + c] = m[v]; qp[v * vstr + c] = pl[v]; }

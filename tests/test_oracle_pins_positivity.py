@@ -1,8 +1,11 @@
 """Pin P18 of the CPU oracle: the positivity fallback of the fifth-order reconstructions (reading C5.1;
 oracle/orc.cpp block_fluxes).  The paper's App. B never discusses positivity of the reconstructed face
-values; the reading taken is: if the reconstructed rho or u at EITHER face of a cell is <= its floor (rho_flr, and
-rho_flr * eps_flr for u, both evaluated at the centre of the cell), that cell falls back to piecewise constant in that
-direction for ALL variables; piecewise-linear reconstructions never take the branch.
+values; the reading taken is: if the reconstructed rho or u at EITHER face of a cell is below its floor (rho_flr, and
+rho_flr * eps_flr for u, both evaluated at the centre of the cell, both lowered by one part in 1e12), that cell falls
+back to piecewise constant in that direction for ALL variables; piecewise-linear reconstructions never take the branch.
+The 1e-12 keeps the decision away from the value the floors themselves produce: con2prim holds whole regions exactly at
+the floor, every reconstruction returns the floor there up to rounding, and a threshold at the floor itself would be decided
+by the last bit of whoever does the arithmetic (the CUDA path evaluates WENO5-Z in a different but equivalent form).
 
 What is checked here is the branch logic, on hand-built stencils whose WENO5-Z face values are worked out by hand:
 which cells fall back, in which direction, for which variables, at which threshold.  The reconstruction itself
@@ -77,8 +80,9 @@ def flagged(p, prim, rfl, ufl):
     """The reading itself, written once more on the pinned face values: allocated indices of the cells that fall back."""
     line, qm, qp = face_states(p, prim)
     g, n = p["ng"], p["nx"]
+    tr, tu = rfl * (1.0 - 1e-12), ufl * (1.0 - 1e-12)
     return [i for i in range(g - 1, g + n + 1)
-            if qm[0, i] <= rfl or qp[0, i] <= rfl or qm[4, i] <= ufl or qp[4, i] <= ufl]
+            if qm[0, i] < tr or qp[0, i] < tr or qm[4, i] < tu or qp[4, i] < tu]
 
 
 def check_line(p, prim, expect_cells):
@@ -147,7 +151,7 @@ def test_p18_density_flux_of_states_at_rest_is_the_closed_form(recon):
         assert abs(F2[0, c] - F[0, c]) > 1e-3
 
 
-def test_p18_threshold_is_less_or_equal_and_u_is_measured_against_rho_floor_times_eps_floor():
+def test_p18_threshold_sits_just_below_the_floor_and_u_is_measured_against_rho_floor_times_eps_floor():
     recon = wl.RECON_WENO5Z
     rho = np.full_like(V, 2.0)
     base = line_params(len(V), recon)
@@ -162,16 +166,32 @@ def test_p18_threshold_is_less_or_equal_and_u_is_measured_against_rho_floor_time
     # u floor 0.56 < 0.6083: not taken, although u < rho_flr
     p = dict(base, rho_floor=1.4, eps_floor=0.4)
     check_line(p, prim, [])
-    # equality counts: floor exactly at the reconstructed value (eps_flr = 1 keeps the product exact)
-    p = dict(base, rho_floor=float(qp[c]), eps_floor=1.0)
-    check_line(p, prim, [c])
-    p = dict(base, rho_floor=float(np.nextafter(qp[c], 0.0)), eps_floor=1.0)
-    check_line(p, prim, [])
+    # a value AT the floor (or within rounding of it) does not count, one that is 2e-12 below it does
+    # (eps_flr = 1 keeps the product exact)
+    for fl, cells in ((float(qp[c]), []), (float(qp[c]) * (1.0 + 1e-15), []), (float(qp[c]) * (1.0 + 5e-13), []),
+                      (float(qp[c]) * (1.0 + 2e-12), [c])):
+        check_line(dict(base, rho_floor=fl, eps_floor=1.0), prim, cells)
     # the same for the density: dip in rho, u far above rho_flr * eps_flr
     prim = line_prims(base, V, np.full_like(V, 3.0), extra=True)
     qm, qp = orc.recon_line(recon, prim[0, 0, 0, 0, :])
-    check_line(dict(base, rho_floor=float(qp[c]), eps_floor=1e-3), prim, [c])
-    check_line(dict(base, rho_floor=float(np.nextafter(qp[c], 0.0)), eps_floor=1e-3), prim, [])
+    for fl, cells in ((float(qp[c]), []), (float(qp[c]) * (1.0 + 5e-13), []), (float(qp[c]) * (1.0 + 2e-12), [c])):
+        check_line(dict(base, rho_floor=fl, eps_floor=1e-3), prim, cells)
+
+
+def test_p18_a_region_held_at_the_floor_keeps_its_reconstruction():
+    """What the 1e-12 is for: cells that con2prim floored carry rho = rho_flr exactly; in a run of such cells WENO5-Z returns
+    rho_flr (1 +- a few 1e-16).  None of them may fall back, whichever way the last bit went."""
+    recon = wl.RECON_WENO5Z
+    fl = 0.3
+    rho = np.array([1.0, 0.9, 0.7, fl, fl, fl, fl, fl, fl, 0.8, 1.1, 1.0, 1.0])
+    p = line_params(len(rho), recon, rho_floor=fl, eps_floor=1e-3)
+    prim = line_prims(p, rho, np.full_like(rho, 3.0), extra=True)
+    line, qm, qp = face_states(p, prim)
+    g = p["ng"]
+    inner = slice(g + 5, g + 7)                           # cells whose whole stencil is at the floor
+    assert np.abs(qm[0, inner] / fl - 1.0).max() < 1e-15 and np.abs(qp[0, inner] / fl - 1.0).max() < 1e-15
+    check_line(p, prim, flagged(p, prim, fl, fl * 1e-3))
+    assert not set(range(g + 3, g + 9)) & set(flagged(p, prim, fl, fl * 1e-3))
 
 
 @pytest.mark.parametrize("recon", FIFTH)
@@ -215,10 +235,10 @@ def test_p18_position_dependent_floor_is_taken_at_the_centre_of_the_cell():
     line, qm, qp = face_states(p, prim)
     x_all = p["xmin"][0] + (np.arange(-p["ng"], p["nx"] + p["ng"]) + 0.5) * dx
     fl_centre = p["rho_floor"] / x_all ** al
-    assert abs(fl_centre[c] - 0.55) < 1e-14 and qp[0, c] <= fl_centre[c]
+    assert abs(fl_centre[c] - 0.55) < 1e-14 and qp[0, c] < fl_centre[c] * (1 - 1e-12)
     assert qp[0, c] > p["rho_floor"] / (xc + 0.5 * dx) ** al
     want_cells = [i for i in range(p["ng"] - 1, p["ng"] + p["nx"] + 1)
-                  if min(qm[0, i], qp[0, i]) <= fl_centre[i] or min(qm[4, i], qp[4, i]) <= fl_centre[i] * 1e-3]
+                  if min(qm[0, i], qp[0, i]) < fl_centre[i] * (1 - 1e-12) or min(qm[4, i], qp[4, i]) < fl_centre[i] * 1e-3 * (1 - 1e-12)]
     assert want_cells[0] == c
     check_line(p, prim, want_cells)
     # one cell further from the origin the same face value would be above the (smaller) floor: the constant form differs
