@@ -94,24 +94,11 @@ __device__ __forceinline__ void face_flux(const MeshDev& m, const Geo<METRIC>& G
 template <int NS>
 __device__ __forceinline__ int hydro_var(int h) { return h < 5 ? h : XS; }   // h-th accumulated component -> variable index
 
-// Every kernel of a stage walks a VIRTUAL grid of tiles (vg.nx x vg.ny x vg.nz, x fastest) with its physical thread blocks
-// striding over it: launched with as many blocks as tiles it is the plain one-tile-per-block launch; launched with a few
-// blocks per SM it is a persistent kernel that leaves room on every SM for the blocks of another kernel (the pipelined
-// stage runs the fp64-bound sweeps of one slab beside the HBM-bound update of the slab before it).
-struct VGrid { unsigned nx, ny, nz; };
-#define PHX_FOR_TILES(vg, bx, by, bz)                                                              \
-  for (unsigned vt_ = blockIdx.x, vn_ = (vg).nx * (vg).ny * (vg).nz; vt_ < vn_; vt_ += gridDim.x)  \
-    if (const unsigned bx = vt_ % (vg).nx, vq_ = vt_ / (vg).nx, by = vq_ % (vg).ny, bz = vq_ / (vg).ny; true)
-
-// Slab of k-planes a launch works on: the x / y sweeps compute the planes kfirst .. kfirst + vg.ny - 1 but add to the
-// divergence accumulator only in the planes kown0 .. kown1 they own (a pipelined slab also computes the plane below it,
-// whose magnetic fluxes its flux-CT needs before the slab that owns that plane has run).
 template <int METRIC, int RECON, int NS>
-__device__ __forceinline__ void sweep_x_tile(const MeshDev& m, const double* __restrict__ prim, double* __restrict__ flux,
-                                             double* __restrict__ racc, int store_all, int nplane, int rowlen, int j0, int k0,
-                                             int kown0, int kown1, unsigned bx, unsigned by, unsigned bz) {
-  // bz = block, by = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii);
-  // consecutive tiles overlap by two positions: thread 0 only supplies the left state of thread 1's face, the last
+__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : (RECON <= 2 ? 5 : PHX_XS_MINB))) k_sweep_x(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+                                                      double* __restrict__ racc, int store_all, int nplane, int rowlen, int j0, int k0) {
+  // blockIdx.z = block, blockIdx.y = kk selects one k-plane; positions inside the plane are tiled flat over (jj, ii);
+  // consecutive thread blocks overlap by two positions: thread 0 only supplies the left state of thread 1's face, the last
   // thread only the upper face of the cell before it
   constexpr int HW = ReconTraits<RECON>::HW;
   constexpr int NQ = NV + NS;
@@ -119,14 +106,14 @@ __device__ __forceinline__ void sweep_x_tile(const MeshDev& m, const double* __r
   __shared__ double sh[NQ][XS_BLOCK];
   __shared__ double shF[NH][XS_BLOCK];
   const int t = threadIdx.x;
-  const int p = bx * (XS_BLOCK - 2) + t;
+  const int p = blockIdx.x * (XS_BLOCK - 2) + t;
   const bool valid = p < nplane;
   double qm[NQ], qp[NQ];
   long long base = 0;
   int ii = 0, i = 0, j = 0, k = 0;
-  const int b = bz;
+  const int b = blockIdx.z;
   if (valid) {
-    const int kk = by;
+    const int kk = blockIdx.y;
     const int jj = p / rowlen;
     ii = p - jj * rowlen;
     i = m.g[0] - 1 + ii; j = j0 + jj; k = k0 + kk;
@@ -176,21 +163,12 @@ __device__ __forceinline__ void sweep_x_tile(const MeshDev& m, const double* __r
     flux[base + BY * m.ncell] = F[BY];
     flux[base + BZ * m.ncell] = F[BZ];
   }
-  // cell (i, j, k): interior along x (ii <= n) and in the transverse directions, in a plane this launch owns
-  if (ii <= m.n[0] && j >= m.g[1] && j < m.g[1] + m.n[1] && k >= kown0 && k <= kown1) {
+  // cell (i, j, k): interior along x (ii <= n) and in the transverse directions
+  if (ii <= m.n[0] && j >= m.g[1] && j < m.g[1] + m.n[1] && k >= m.g[2] && k < m.g[2] + m.n[2]) {
     const long long rb = (long long)b * NH * m.ncell + (long long)k * m.sk + (long long)j * m.sj + i;
 #pragma unroll
     for (int h = 0; h < NH; ++h) racc[rb + h * m.ncell] = 0.0 - (shF[h][t + 1] - F[hydro_var<NS>(h)]) * m.rdx[0];
   }
-}
-
-template <int METRIC, int RECON, int NS>
-__global__ void __launch_bounds__(XS_BLOCK, (RECON == 4 ? 6 : (RECON <= 2 ? 5 : PHX_XS_MINB))) k_sweep_x(MeshDev m, VGrid vg, const double* __restrict__ prim, double* __restrict__ flux,
-                                                      double* __restrict__ racc, int store_all, int nplane, int rowlen, int j0, int k0,
-                                                      int kown0, int kown1) {
-  // a tile's shared arrays are free for the next tile: whoever is past the second barrier of a tile has seen every thread
-  // finish reading sh, and shF is written only after the first barrier of the next tile
-  PHX_FOR_TILES(vg, bx, by, bz) sweep_x_tile<METRIC, RECON, NS>(m, prim, flux, racc, store_all, nplane, rowlen, j0, k0, kown0, kown1, bx, by, bz);
 }
 
 // ---- y / z sweep ---------------------------------------------------------------------------------
@@ -209,42 +187,35 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// March range: the launch covers the cells cfirst .. clast along D (the whole interior, or one slab of a z sweep) in
-// segments of L cells, and the transverse positions o = lo1 .. of which oown0 .. oown1 are owned (divergence accumulated).
-// Faces: a segment computes f0 .. c1+1 and stores f0 .. c1; the face clast+1 is stored by the last segment, the face cfirst
-// only if store_lo is set (a pipelined slab leaves it to the slab below, which computed it as its own upper end, unless it
-// is the first slab to run in its stage).
-struct MarchRange { int cfirst, clast, L, store_lo, oown0, oown1; };
-
 template <int METRIC, int RECON, int D, int NS>
-__device__ __forceinline__ void sweep_march_tile(const MeshDev& m, const double* __restrict__ prim, double* __restrict__ flux,
-                                                 double* __restrict__ racc, int store_all, int first,
-                                                 int ntr, int n0, int lo0, int lo1, const MarchRange& mr, unsigned bx, unsigned by, unsigned bz) {
+__global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m, const double* __restrict__ prim, double* __restrict__ flux,
+                                                                       double* __restrict__ racc, int store_all, int first,
+                                                                       int ntr, int n0, int lo0, int lo1, int L) {
   constexpr int HW = ReconTraits<RECON>::HW;
   constexpr int NW = 2 * HW + 1;   // stencil rows
   constexpr int NR = NW + 1;       // ring: the stencil plus one row in flight
   constexpr int NQ = NV + NS;
   constexpr int NH = 5 + NS;
+  constexpr int O = (D == 1) ? 2 : 1;   // the other transverse direction
   __shared__ double win[NR][NQ][MS_BLOCK];
   const int tid = threadIdx.x;
-  const int p = bx * MS_BLOCK + tid;
+  const int p = blockIdx.x * MS_BLOCK + tid;
   if (p >= ntr) return;
-  const int b = bz;
-  const int seg = by;
-  const int L = mr.L;
+  const int b = blockIdx.z;
+  const int seg = blockIdx.y;
   const int t1 = p / n0, t0 = p - t1 * n0;
   const int i = lo0 + t0;             // x index
   const int o = lo1 + t1;             // the other transverse index (k for D=1, j for D=2)
   const long long sd = (D == 1) ? m.sj : m.sk;
   const long long so = (D == 1) ? m.sk : m.sj;
-  const int clast = mr.clast;                     // last cell along D of this launch
-  const int f0 = mr.cfirst + seg * L;             // first cell (and first face) of this segment
+  const int clast = m.g[D] + m.n[D] - 1;          // last interior cell along D
+  const int f0 = m.g[D] + seg * L;                // first cell (and first face) of this segment
   const int c1 = min(f0 + L - 1, clast);          // last cell
   if (f0 > c1) return;
   const int f1 = c1 + 1;                          // last face computed here
   const long long col = (long long)b * m.nvar * m.ncell + (long long)o * so + i;
   const long long rcol = (long long)b * NH * m.ncell + (long long)o * so + i;
-  const bool inner = i >= m.g[0] && i < m.g[0] + m.n[0] && o >= mr.oown0 && o <= mr.oown1;   // interior column this launch owns
+  const bool inner = i >= m.g[0] && i < m.g[0] + m.n[0] && o >= m.g[O] && o < m.g[O] + m.n[O];   // interior column
   int cb[3];
   block_coords(m, b, cb);
   const double xx = xcen(m, 0, cb[0], i);
@@ -318,7 +289,7 @@ __device__ __forceinline__ void sweep_march_tile(const MeshDev& m, const double*
       if (D == 1) G.at(m, xx, xf, xo); else G.at(m, xx, xo, xf);
       double F[NQ];
       face_flux<METRIC, D, NS>(m, G, qpPrev, qm, F);
-      if ((c <= c1 || c == clast + 1) && (c > mr.cfirst || mr.store_lo)) {   // c1+1 is stored by the next segment unless it is the last face
+      if (c <= c1 || c == clast + 1) {            // the face c1+1 is stored by the next segment unless it is the last face
         if (store_all) {
 #pragma unroll
           for (int v = 0; v < NQ; ++v) flux[col + v * m.ncell + (long long)c * sd] = F[v];
@@ -348,14 +319,6 @@ __device__ __forceinline__ void sweep_march_tile(const MeshDev& m, const double*
     snew = (snew + 1 == NR) ? 0 : snew + 1;
   }
   cp_async_wait<0>();
-}
-
-template <int METRIC, int RECON, int D, int NS>
-__global__ void __launch_bounds__(MS_BLOCK, PHX_MS_MINB) k_sweep_march(MeshDev m, VGrid vg, const double* __restrict__ prim, double* __restrict__ flux,
-                                                                       double* __restrict__ racc, int store_all, int first,
-                                                                       int ntr, int n0, int lo0, int lo1, MarchRange mr) {
-  // a thread touches only its own column of the shared ring, so tiles need no barrier between them
-  PHX_FOR_TILES(vg, bx, by, bz) sweep_march_tile<METRIC, RECON, D, NS>(m, prim, flux, racc, store_all, first, ntr, n0, lo0, lo1, mr, bx, by, bz);
 }
 
 // ---- update: flux-CT + divergence + sources + RK combine + con2prim + floors ----------------------
@@ -393,19 +356,16 @@ template <int METRIC, bool EXC, bool CFL, int NS, bool RF>
 __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                               double bdt_host, const double* __restrict__ d_dt, double beta,
                                               const double* cons0, const double* cons_in, double* cons_out,
-                                              const double* prim_in, double* prim, unsigned char* __restrict__ mask,
-                                              int kk0, unsigned bx, unsigned by, unsigned bz) {
+                                              double* __restrict__ prim, unsigned char* __restrict__ mask) {
   // U~_out = g0 U~0 + g1 U~_in + bdt R.  cons_out may alias cons_in or cons0 (every thread touches only its own cell of
-  // the conserved fields); cons_in is not read when g1 == 0 (first stage).  prim_in: the stage-input primitives; prim: where
-  // the new ones go (the same field, or the second primitive field of a pipelined stage: then the sweeps of other slabs
-  // still read prim_in while this slab is updated).
-  // bz = block, by + kk0 = kk selects one interior k-plane; the plane is tiled flat over (jj, ii)
-  const int p = bx * UP_BLOCK + threadIdx.x;
+  // the conserved fields); cons_in is not read when g1 == 0 (first stage).
+  // blockIdx.z = block, blockIdx.y = kk selects one interior k-plane; the plane is tiled flat over (jj, ii)
+  const int p = blockIdx.x * UP_BLOCK + threadIdx.x;
   if (p >= m.n[0] * m.n[1]) return 0.0;
   const int jj = p / m.n[0];
   const int ii = p - jj * m.n[0];
-  const int b = bz;
-  const int kk = by + kk0;
+  const int b = blockIdx.z;
+  const int kk = blockIdx.y;
   const int i = ii + m.g[0], j = jj + m.g[1], k = kk + m.g[2];
   const long long c = (long long)k * m.sk + (long long)j * m.sj + i;
   constexpr int NQ = NV + NS;
@@ -417,7 +377,6 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
       for (int v = 0; v < NQ; ++v) {
         const long long id = vb + v * m.ncell + c;
         cons_out[id] = (g1 != 0.0) ? g0 * cons0[id] + g1 * cons_in[id] : cons0[id];
-        if (prim != prim_in) prim[id] = prim_in[id];
       }
       mask[fb + c] = M_EXCISED;
       return 0.0;
@@ -440,7 +399,7 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
     }
     if constexpr (STG == 1) {
 #pragma unroll
-      for (int v = 0; v < NPQ; ++v) cp_async8(&stg[2 * NQ + v][tid], prim_in + vb + v * m.ncell + c);
+      for (int v = 0; v < NPQ; ++v) cp_async8(&stg[2 * NQ + v][tid], prim + vb + v * m.ncell + c);
     }
     cp_async_commit();
   }
@@ -485,10 +444,10 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
 #pragma unroll
     for (int v = 0; v < NPQ; ++v) q[v] = stg[2 * NQ + v][tid];
   } else {
-    q[RHO] = prim_in[vb + RHO * m.ncell + c];
-    q[UX] = prim_in[vb + UX * m.ncell + c]; q[UY] = prim_in[vb + UY * m.ncell + c]; q[UZ] = prim_in[vb + UZ * m.ncell + c];
-    q[UU] = prim_in[vb + UU * m.ncell + c];
-    if constexpr (METRIC == 1) { q[BX] = prim_in[vb + BX * m.ncell + c]; q[BY] = prim_in[vb + BY * m.ncell + c]; q[BZ] = prim_in[vb + BZ * m.ncell + c]; }
+    q[RHO] = prim[vb + RHO * m.ncell + c];
+    q[UX] = prim[vb + UX * m.ncell + c]; q[UY] = prim[vb + UY * m.ncell + c]; q[UZ] = prim[vb + UZ * m.ncell + c];
+    q[UU] = prim[vb + UU * m.ncell + c];
+    if constexpr (METRIC == 1) { q[BX] = prim[vb + BX * m.ncell + c]; q[BY] = prim[vb + BY * m.ncell + c]; q[BZ] = prim[vb + BZ * m.ncell + c]; }
   }
   if constexpr (METRIC == 1) {
     double S[4];
@@ -531,14 +490,12 @@ __device__ __forceinline__ double update_cell(const MeshDev& m, const FluxPtrs& 
 // orders like the unsigned integer), one atomicMax per thread block; k_cfl_final_slots turns them into the time step.
 constexpr int PHX_NSLOT = 1024;
 template <int METRIC, bool EXC, bool CFL, int NS, bool RF>
-__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 1 ? PHX_UP_MINB_KS : PHX_UP_MINB)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,  // tiles: (plane tile, k-plane, block)
+__global__ void __launch_bounds__(UP_BLOCK, (METRIC == 1 ? PHX_UP_MINB_KS : PHX_UP_MINB)) k_update(MeshDev m, FluxPtrs fl, const unsigned char* __restrict__ xfl, double g0, double g1,
                                                      double bdt_host, const double* __restrict__ d_dt, double beta,
                                                      const double* cons0, const double* cons_in, double* cons_out,
-                                                     const double* prim_in, double* prim, unsigned char* __restrict__ mask,
-                                                     unsigned long long* __restrict__ smax, VGrid vg, int kk0) {
-  double sum = 0.0;
-  PHX_FOR_TILES(vg, bx, by, bz)
-    sum = fmax(sum, update_cell<METRIC, EXC, CFL, NS, RF>(m, fl, xfl, g0, g1, bdt_host, d_dt, beta, cons0, cons_in, cons_out, prim_in, prim, mask, kk0, bx, by, bz));
+                                                     double* __restrict__ prim, unsigned char* __restrict__ mask,
+                                                     unsigned long long* __restrict__ smax) {
+  double sum = update_cell<METRIC, EXC, CFL, NS, RF>(m, fl, xfl, g0, g1, bdt_host, d_dt, beta, cons0, cons_in, cons_out, prim, mask);
   if constexpr (CFL) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sum = fmax(sum, __shfl_xor_sync(0xffffffffu, sum, o));
@@ -549,7 +506,7 @@ __global__ void __launch_bounds__(UP_BLOCK, (METRIC == 1 ? PHX_UP_MINB_KS : PHX_
       double v = sh[0];
 #pragma unroll
       for (int w = 1; w < UP_BLOCK / 32; ++w) v = fmax(v, sh[w]);
-      const unsigned slot = blockIdx.x % PHX_NSLOT;
+      const unsigned slot = (blockIdx.x + blockIdx.y * gridDim.x + blockIdx.z * gridDim.x * gridDim.y) % PHX_NSLOT;
       atomicMax(&smax[slot], (unsigned long long)__double_as_longlong(v));
     }
   }
@@ -635,27 +592,25 @@ __global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* _
 }
 
 // ---- ghost fill: one gather pass -------------------------------------------------------------------
-// blockIdx.z = block; the threads enumerate the ghost cells of the block only: first the full k-planes below the interior
-// (nAlo cells: 0 or g_z planes) and above it (nAhi cells), then the 2 g_y full rows of the interior k-planes kk0 .. kk0+nkk-1,
-// then the 2 g_x end cells of every interior row of those planes (nB: size of the row group, ntot: all cells enumerated).
-// The whole frame is nAlo = nAhi = g_z planes, kk0 = 0, nkk = n_z; a pipelined stage fills the frame slab by slab.
-__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, int nAlo, int nAhi, int nB, int ntot, int kk0) {
+// blockIdx.z = block; the threads enumerate the ghost cells of the block only: first the 2 g_z full k-planes, then the
+// 2 g_y full rows of every interior k-plane, then the 2 g_x end cells of every interior row (nA, nB: sizes of the first
+// two groups, ntot: all ghost cells of one block).
+__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, int nA, int nB, int ntot) {
   int t = blockIdx.x * 256 + threadIdx.x;
   if (t >= ntot) return;
   int l[3];
-  const int nA = nAlo + nAhi;
   if (t < nA) {
     const int plane = m.na[0] * m.na[1];
-    int kz;
-    if (t < nAlo) { kz = t / plane; t -= kz * plane; l[2] = kz; }
-    else { t -= nAlo; kz = t / plane; t -= kz * plane; l[2] = m.g[2] + m.n[2] + kz; }
+    const int kz = t / plane;
+    t -= kz * plane;
+    l[2] = kz < m.g[2] ? kz : kz + m.n[2];
     l[1] = t / m.na[0];
     l[0] = t - l[1] * m.na[0];
   } else if (t < nA + nB) {
     t -= nA;
     const int per = 2 * m.g[1] * m.na[0];
-    const int kk = kk0 + t / per;
-    t -= (kk - kk0) * per;
+    const int kk = t / per;
+    t -= kk * per;
     const int jy = t / m.na[0];
     l[2] = m.g[2] + kk;
     l[1] = jy < m.g[1] ? jy : jy + m.n[1];
@@ -666,7 +621,7 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restri
     const int row = t / w;
     const int ix = t - row * w;
     const int kk = row / m.n[1];
-    l[2] = m.g[2] + kk0 + kk;
+    l[2] = m.g[2] + kk;
     l[1] = m.g[1] + (row - kk * m.n[1]);
     l[0] = ix < m.g[0] ? ix : ix + m.n[0];
   }
@@ -978,12 +933,17 @@ extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* str
   return PHX_OK;
 }
 
+// PHX_BUILD_SUBSET (development only): instantiate the flat-metric WENO5-Z / PLM kernels alone, for quick A/B builds
+#ifdef PHX_BUILD_SUBSET
+#define DISPATCH_METRIC(mesh, CALL) do { CALL(0); } while (0)
+#else
 #define DISPATCH_METRIC(mesh, CALL)                 \
   do {                                              \
     if ((mesh)->m.metric == 0) { CALL(0); }         \
     else if ((mesh)->m.metric == 1) { CALL(1); }    \
     else { CALL(2); }                               \
   } while (0)
+#endif
 
 extern "C" int phx_prim_to_cons(const phx_mesh* M, const double* d_prim, double* d_cons, void* stream) {
   if (!M || !aligned16(d_prim) || !aligned16(d_cons)) return fail(PHX_EINVAL, "phx_prim_to_cons: null or misaligned argument");
@@ -999,23 +959,14 @@ extern "C" int phx_prim_to_cons(const phx_mesh* M, const double* d_prim, double*
   return PHX_OK;
 }
 
-// ghost cells of the k-planes below (zlo) / above (zhi) the interior and the x / y ghosts of the interior planes kk0 .. kk0+nkk-1
-static void launch_fill_ghosts(const phx_mesh* M, double* d_prim, bool zlo, bool zhi, int kk0, int nkk, cudaStream_t st) {
-  const MeshDev& m = M->m;
-  const long long plane = (long long)m.g[2] * m.na[1] * m.na[0];
-  const long long nAlo = zlo ? plane : 0, nAhi = zhi ? plane : 0;
-  const long long nB = 2LL * nkk * m.g[1] * m.na[0], nC = 2LL * nkk * m.n[1] * m.g[0];
-  const long long ntot = nAlo + nAhi + nB + nC;
-  if (ntot == 0) return;
-  const dim3 grid((unsigned)((ntot + 255) / 256), 1, m.nblk);
-  k_fill_ghosts<<<grid, 256, 0, st>>>(m, d_prim, (int)nAlo, (int)nAhi, (int)nB, (int)ntot, kk0);
-}
-
 extern "C" int phx_fill_ghosts(const phx_mesh* M, double* d_prim, void* stream) {
   if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
   if (M->nall == M->ninterior) return PHX_OK;
   { ProfScope ps(M, PHX_K_FILL_GHOSTS, (cudaStream_t)stream);
-    launch_fill_ghosts(M, d_prim, true, true, 0, M->m.n[2], (cudaStream_t)stream); }
+    const MeshDev& m = M->m;
+    const long long nA = 2LL * m.g[2] * m.na[1] * m.na[0], nB = 2LL * m.n[2] * m.g[1] * m.na[0], nC = 2LL * m.n[2] * m.n[1] * m.g[0];
+    const dim3 grid((unsigned)((nA + nB + nC + 255) / 256), 1, m.nblk);
+    k_fill_ghosts<<<grid, 256, 0, (cudaStream_t)stream>>>(m, d_prim, (int)nA, (int)nB, (int)(nA + nB + nC)); }
   LAUNCH_CHECK(M, "k_fill_ghosts");
   return PHX_OK;
 }
@@ -1044,47 +995,20 @@ extern "C" int phx_cons_to_prim(const phx_mesh* M, double* d_cons, double* d_pri
 }
 
 // ---- sweeps -------------------------------------------------------------------------------------------------
-// What part of the mesh one group of launches works on, and with how many thread blocks.
-struct Slab {
-  int kk0, nkk;             // interior k-planes owned (0-based inside the interior); the whole mesh is (0, n_z)
-  int halo_lo, halo_hi;     // the x / y sweeps also compute this many planes below / above (flux-CT reads the magnetic fluxes one plane beyond)
-  int store_lo;             // the z sweep stores the face under the slab's first plane
-  int sweep_blocks;         // thread blocks per sweep launch; 0 = one per tile
-  int update_blocks;        // thread blocks of the update launch; 0 = one per tile
-};
-static Slab whole_mesh(const MeshDev& m) {
-  Slab s;
-  s.kk0 = 0; s.nkk = m.n[2];
-  s.halo_lo = s.halo_hi = m.act[2] ? 1 : 0;
-  s.store_lo = 1; s.sweep_blocks = 0; s.update_blocks = 0;
-  return s;
-}
-static unsigned tiles_of(const VGrid& vg) { return vg.nx * vg.ny * vg.nz; }
-static unsigned blocks_for(const VGrid& vg, int limit) {
-  const unsigned t = tiles_of(vg);
-  return (limit > 0 && (unsigned)limit < t) ? (unsigned)limit : t;
-}
-
-// which: bit 0 x sweep, bit 1 y sweep, bit 2 z sweep
 template <int METRIC, int RECON, int NS>
-static void launch_sweeps_t(phx_mesh* M, const double* prim, const Slab& sl, int which, cudaStream_t st) {
+static void launch_sweeps_t(phx_mesh* M, const double* prim, cudaStream_t st) {
   const MeshDev& m = M->m;
   int lo[3], cnt[3];
   for (int d = 0; d < 3; ++d) {
     lo[d] = m.act[d] ? m.g[d] - 1 : 0;
     cnt[d] = m.act[d] ? m.n[d] + 2 : 1;
   }
-  // k-planes of the x and y sweeps, and the ones whose divergence they own
-  const int kfirst = m.act[2] ? m.g[2] + sl.kk0 - sl.halo_lo : 0;
-  const int nk = m.act[2] ? sl.nkk + sl.halo_lo + sl.halo_hi : 1;
-  const int kown0 = m.g[2] + sl.kk0, kown1 = kown0 + sl.nkk - 1;
-  if (m.act[0] && (which & 1)) {
+  if (m.act[0]) {
     const int rowlen = m.n[0] + 2;
     const int nplane = cnt[1] * rowlen;
-    VGrid vg = {(unsigned)((nplane - 1 + (XS_BLOCK - 3)) / (XS_BLOCK - 2)), (unsigned)nk, (unsigned)m.nblk};   // every position >= 1 is some tile's thread 1..XS_BLOCK-2
+    dim3 grid((nplane - 1 + (XS_BLOCK - 3)) / (XS_BLOCK - 2), cnt[2], m.nblk);   // every position >= 1 is some block's thread 1..XS_BLOCK-2
     ProfScope ps(M, PHX_K_SWEEP_X, st);
-    k_sweep_x<METRIC, RECON, NS><<<blocks_for(vg, sl.sweep_blocks), XS_BLOCK, 0, st>>>(m, vg, prim, M->flux[0], M->racc, M->store_all_fluxes, nplane, rowlen,
-                                                                                       lo[1], kfirst, kown0, kown1);
+    k_sweep_x<METRIC, RECON, NS><<<grid, XS_BLOCK, 0, st>>>(m, prim, M->flux[0], M->racc, M->store_all_fluxes, nplane, rowlen, lo[1], lo[2]);
     M->launches++;
   }
   // Segments of at most 33 faces along the sweep direction; a small mesh gets more, shorter segments (at least 4 faces)
@@ -1100,54 +1024,56 @@ static void launch_sweeps_t(phx_mesh* M, const double* prim, const Slab& sl, int
     if (need > nseg) nseg = need < cap ? need : cap;
     return nseg < 1 ? 1 : nseg;
   };
-  if (m.act[1] && (which & 2)) {
+  if (m.act[1]) {
     const int ncells = m.n[1];
-    const int ntr = cnt[0] * nk;
+    const int ntr = cnt[0] * cnt[2];
     const int nseg = segments(ncells, ntr);
-    MarchRange mr = {m.g[1], m.g[1] + m.n[1] - 1, (ncells + nseg - 1) / nseg, 1, kown0, kown1};
-    VGrid vg = {(unsigned)((ntr + MS_BLOCK - 1) / MS_BLOCK), (unsigned)nseg, (unsigned)m.nblk};
+    const int L = (ncells + nseg - 1) / nseg;
+    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Y, st);
-    k_sweep_march<METRIC, RECON, 1, NS><<<blocks_for(vg, sl.sweep_blocks), MS_BLOCK, 0, st>>>(m, vg, prim, M->flux[1], M->racc, M->store_all_fluxes, m.act[0] ? 0 : 1,
-                                                                                              ntr, cnt[0], lo[0], kfirst, mr);
+    k_sweep_march<METRIC, RECON, 1, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[1], M->racc, M->store_all_fluxes, m.act[0] ? 0 : 1, ntr, cnt[0], lo[0], lo[2], L);
     M->launches++;
   }
-  if (m.act[2] && (which & 4)) {
-    const int ncells = sl.nkk;
+  if (m.act[2]) {
+    const int ncells = m.n[2];
     const int ntr = cnt[0] * cnt[1];
     const int nseg = segments(ncells, ntr);
-    MarchRange mr = {kown0, kown1, (ncells + nseg - 1) / nseg, sl.store_lo, m.g[1], m.g[1] + m.n[1] - 1};
-    VGrid vg = {(unsigned)((ntr + MS_BLOCK - 1) / MS_BLOCK), (unsigned)nseg, (unsigned)m.nblk};
+    const int L = (ncells + nseg - 1) / nseg;
+    dim3 grid((ntr + MS_BLOCK - 1) / MS_BLOCK, nseg, m.nblk);
     ProfScope ps(M, PHX_K_SWEEP_Z, st);
-    k_sweep_march<METRIC, RECON, 2, NS><<<blocks_for(vg, sl.sweep_blocks), MS_BLOCK, 0, st>>>(m, vg, prim, M->flux[2], M->racc, M->store_all_fluxes,
-                                                                                              (m.act[0] || m.act[1]) ? 0 : 1, ntr, cnt[0], lo[0], lo[1], mr);
+    k_sweep_march<METRIC, RECON, 2, NS><<<grid, MS_BLOCK, 0, st>>>(m, prim, M->flux[2], M->racc, M->store_all_fluxes, (m.act[0] || m.act[1]) ? 0 : 1, ntr, cnt[0], lo[0], lo[1], L);
     M->launches++;
   }
 }
 
-static void launch_sweeps(phx_mesh* M, const double* prim, const Slab& sl, int which, cudaStream_t st) {
+static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
   const int key = M->m.metric * 6 + M->m.recon;
   switch (key) {
-#define PHX_CASE(MET, REC) case MET * 6 + REC: if (M->m.nvar == NV) launch_sweeps_t<MET, REC, 0>(M, prim, sl, which, st); else launch_sweeps_t<MET, REC, 1>(M, prim, sl, which, st); break;
+#define PHX_CASE(MET, REC) case MET * 6 + REC: if (M->m.nvar == NV) launch_sweeps_t<MET, REC, 0>(M, prim, st); else launch_sweeps_t<MET, REC, 1>(M, prim, st); break;
+#ifdef PHX_BUILD_SUBSET
+    PHX_CASE(0, 1) PHX_CASE(0, 3)
+#else
     PHX_CASE(0, 0) PHX_CASE(0, 1) PHX_CASE(0, 2) PHX_CASE(0, 3) PHX_CASE(0, 4) PHX_CASE(0, 5)
     PHX_CASE(1, 0) PHX_CASE(1, 1) PHX_CASE(1, 2) PHX_CASE(1, 3) PHX_CASE(1, 4) PHX_CASE(1, 5)
     PHX_CASE(2, 0) PHX_CASE(2, 1) PHX_CASE(2, 2) PHX_CASE(2, 3) PHX_CASE(2, 4) PHX_CASE(2, 5)
+#endif
 #undef PHX_CASE
     default: break;
   }
 }
 
-// flux-CT + update + con2prim + floors of the k-planes of `sl`; prim_in: stage input, prim_out: where the new primitives go
-static int launch_update(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
-                         const double* d_cons_in, double* d_cons_out, const double* prim_in, double* prim_out, unsigned char* d_mask,
-                         const Slab& sl, bool reduce_cfl, cudaStream_t st) {
+static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
+                      const double* d_cons_in, double* d_cons_out, double* d_prim, unsigned char* d_mask, cudaStream_t st,
+                      bool reduce_cfl = false) {
+  launch_sweeps(M, d_prim, st);
+  { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
   FluxPtrs fl;
   for (int d = 0; d < 3; ++d) fl.f[d] = M->flux[d];
   fl.racc = M->racc;
-  VGrid vg = {(unsigned)((M->m.n[0] * M->m.n[1] + UP_BLOCK - 1) / UP_BLOCK), (unsigned)sl.nkk, (unsigned)M->m.nblk};
-  const unsigned nb = blocks_for(vg, sl.update_blocks);
+  const dim3 nb((M->m.n[0] * M->m.n[1] + UP_BLOCK - 1) / UP_BLOCK, M->m.n[2], M->m.nblk);
   {
   ProfScope ps(M, PHX_K_UPDATE, st);
-#define UPD(MET, EXC, CFLR, NSC, RFL) k_update<MET, EXC, CFLR, NSC, RFL><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, prim_in, prim_out, d_mask, M->smax, vg, sl.kk0)
+#define UPD(MET, EXC, CFLR, NSC, RFL) k_update<MET, EXC, CFLR, NSC, RFL><<<nb, UP_BLOCK, 0, st>>>(M->m, fl, M->xfl, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_mask, M->smax)
 #define UPD2(MET, NSC, RFL)                                                                                  \
   if (M->m.excise) { if (reduce_cfl) UPD(MET, true, true, NSC, RFL); else UPD(MET, true, false, NSC, RFL); } \
   else { if (reduce_cfl) UPD(MET, false, true, NSC, RFL); else UPD(MET, false, false, NSC, RFL); }
@@ -1160,17 +1086,6 @@ static int launch_update(phx_mesh* M, double g0, double g1, double bdt_host, con
 #undef UPD
   }
   LAUNCH_CHECK(M, "k_update");
-  return PHX_OK;
-}
-
-static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
-                      const double* d_cons_in, double* d_cons_out, double* d_prim, unsigned char* d_mask, cudaStream_t st,
-                      bool reduce_cfl = false) {
-  const Slab all = whole_mesh(M->m);
-  launch_sweeps(M, d_prim, all, 7, st);
-  { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
-  const int rc = launch_update(M, g0, g1, bdt_host, d_dt, beta, d_cons0, d_cons_in, d_cons_out, d_prim, d_prim, d_mask, all, reduce_cfl, st);
-  if (rc != PHX_OK) return rc;
   return phx_fill_ghosts(M, d_prim, st);
 }
 
