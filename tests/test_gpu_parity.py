@@ -134,6 +134,7 @@ def test_cons_to_prim_floors_and_failure_masks():
     # 1e-8: the inversion's condition number on these extreme states (W up to ~16, eps down to 1e-4, b^2/rho >> 1)
     # is ~1e7-1e8 ulp (2e-9 seen for bisection-vs-exact on such states); config-like states are held
     # to 1e-12 by test_cons_to_prim_matches_oracle
+    print("floors / failure masks: max point-wise relative difference of the primitives", (np.abs(got - ref) / den).max())
     assert (np.abs(got - ref) / den).max() < 1e-8
     cg = interior(p, cons.cpu().numpy()); cr = interior(p, cons_ref)
     fin = np.isfinite(cr)

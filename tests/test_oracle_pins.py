@@ -283,9 +283,11 @@ def test_p6_kerr_schild_identities_and_derivatives():
             assert abs(s["alpha"] * s["sqrtg"] - 1.0) < 1e-13
             assert np.abs(s["gamma_u"] @ s["gamma_l"] - np.eye(3)).max() < 1e-13
             # closed forms: alpha=(1+2H)^-1/2, beta^i = 2H l_i/(1+2H), gamma^ij = delta - 2H l_i l_j/(1+2H)
-            r = wl.ks_radius(*x, a)
-            # r solves r^4 - (R^2-a^2) r^2 - a^2 z^2 = 0
+            # r: the positive root of r^4 - (R^2-a^2) r^2 - a^2 z^2 = 0, from numpy's polynomial solver (no formula of the
+            # shared input module enters a pin)
             R2 = x @ x
+            roots = np.roots([1.0, 0.0, -(R2 - a * a), 0.0, -a * a * x[2] ** 2])
+            r = float(max(t.real for t in roots if abs(t.imag) < 1e-9 and t.real > 0))
             assert abs(r ** 4 - (R2 - a * a) * r * r - a * a * x[2] ** 2) < 1e-10 * r ** 4
             H = r ** 3 / (r ** 4 + a * a * x[2] ** 2)
             l = np.array([(r * x[0] + a * x[1]) / (r * r + a * a), (r * x[1] - a * x[0]) / (r * r + a * a), x[2] / r])
