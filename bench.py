@@ -11,8 +11,11 @@ seeded synthetic fields from paper_2410_09146_b200/workloads.py (recipe in DESIG
 value     : interior zones x K / device time (CUDA events, max over ranks), state resident in HBM.
 e2e       : same metric through phx_evolve_host (HOST buffers: H2D of the primitives and D2H of the new primitives
             and the mask inside the timed region, one call per step).
-roofline  : dominant kernel class, per-launch time from CUDA events recorded by the library on the launching
-            stream inside the timed region (phx_profile_*), algorithmic bytes / flops per zone from DESIGN.md 6.
+roofline  : the dominant kernel class (the three reconstruct + Riemann sweeps, fp64-bound) against the fp64 peak measured in
+            the same run (phx_debug_fp64_peak), per-launch time from CUDA events recorded by the library on the launching
+            stream inside the timed region (phx_profile_*); executed fp64 work and DRAM traffic per launch from the ncu
+            capture named in COUNTS_FILE, used only if it was taken from the kernel sources that run; plus the update
+            kernel against the HBM copy bandwidth and the whole step as SURVEY.md 8(d) defines its roofline.
 cpu_baseline : the oracle (oracle/, as it stands) on a bounded sample of the same workload on the host cores.
 N > 1     : the path does not shard in this build ("replicas only") - every rank runs an independent
             replica of the same workload, no data-path collective; value = N x zones x K / max-over-ranks time.
@@ -34,29 +37,35 @@ if ROOT not in sys.path:
 METRIC = "grmhd_zone_cycles_per_sec"
 UNIT = "zone-cycles/s"
 
-# Algorithmic traffic and arithmetic per interior zone and launch.
-# Bytes: what the kernel's definition must move.  The sweeps read P (64 B), write the two magnetic flux components flux-CT
-# needs (16 B) and accumulate the divergence of the five non-magnetic components (x: 40 B written; y, z: 40 B read + 40 B
-# written).  update = that divergence (40 B) + 3 x 2 magnetic flux components (48 B) + U~0 read + U~1 read (stage 2 only:
-# 32 B averaged over both stages) + 5 primitives read (sources / con2prim guess) + U~ and P written + mask.
+# Algorithmic traffic per interior zone and launch: what the kernel's definition must move.
+# The sweeps read P (64 B), write the two magnetic flux components flux-CT needs (16 B) and accumulate the divergence of the
+# five non-magnetic components (x: 40 B written; y, z: 40 B read + 40 B written).
+# update, two byte models: "design" = everything this design makes the kernel move (the accumulated divergence 40 B + 3 x 2
+# magnetic flux components 48 B + U~0 64 B + U~1 in stage 2 only, 32 B averaged + 5 primitives 40 B + U~ and P written
+# 128 B + mask 1 B = 353 B); "method" = without the two intermediates the split into sweeps and update creates (265 B).
 ALGO_BYTES_PER_ZONE = {
     "sweep_x": 64.0 + 16.0 + 40.0, "sweep_y": 64.0 + 16.0 + 80.0, "sweep_z": 64.0 + 16.0 + 80.0,
     "update": 40.0 + 48.0 + 64.0 + 32.0 + 40.0 + 64.0 + 64.0 + 1.0,
     "fill_ghosts": 0.0, "cfl": 64.0, "prim_to_cons": 128.0, "c2p": 129.0, "copy": 128.0,
 }
-# fp64 flop per interior zone and launch for the WENO5-Z + HLL Minkowski path: dadd + dmul + 2*dfma thread-instructions of
-# the committed kernels counted by ncu (profiles/r01_ncu_summary.md; con2prim iterations are data dependent, the figure
-# is the one measured on this workload).  achieved = these flops / measured time, i.e. useful fp64 work only.
-# update: average of the first stage (631) and the second stage, which also evaluates the signal speeds for the fused CFL
-# reduction (760); the "cfl" class is the one-block final kernel of that reduction
-ALGO_FLOP_PER_ZONE = {"sweep_x": 1106.0, "sweep_y": 1141.0, "sweep_z": 1141.0, "update": 695.0, "cfl": 0.0}
-# fp64 peak from unit counts and clocks: 148 SM x 64 fp64 lanes x 2 flop x 1.965 GHz; a DFMA loop measured
-# 33.9 TFLOP/s on this pool's B200 (16.94 T DFMA/s)
-FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-FP64_MEASURED_DFMA_TFLOPS = 33.9
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (bytes)
-NCU_TRAFFIC = {256: {"update": 6.126e9, "sweep_x": 2.040e9, "sweep_y": 2.797e9, "sweep_z": 2.796e9, "cfl": 0.0,
-                     "fill_ghosts": 0.255e9}}
+UPDATE_METHOD_BYTES_PER_ZONE = 64.0 + 32.0 + 40.0 + 64.0 + 64.0 + 1.0
+# Executed fp64 work per zone and DRAM traffic per launch are NOT constants of this file: they are read from the ncu
+# capture named here (written by paper_2410_09146_b200/profile_counts.py), and used only if the kernel sources this run
+# executes hash to what the capture was taken from.
+COUNTS_FILE = os.path.join("profiles", "r02_kernel_counts.csv")
+COUNTS_WORKLOAD = "cfg4_256"
+SWEEPS = ("sweep_x", "sweep_y", "sweep_z")
+
+
+def load_counts():
+    """({class: counts}, capture id, valid) for the 256^3 bench workload; valid = the capture is of these kernel sources."""
+    from paper_2410_09146_b200 import profile_counts as pc
+    path = os.path.join(ROOT, COUNTS_FILE)
+    if not os.path.exists(path):
+        return {}, None, False
+    rows, sha = pc.load(path, COUNTS_WORKLOAD)
+    cap = next(iter(rows.values()))["capture"] if rows else None
+    return rows, cap, bool(rows) and sha == pc.source_hash()
 
 
 def parse_args():
@@ -131,6 +140,14 @@ def oracle_cores():
         return len(os.sched_getaffinity(0))
     except AttributeError:
         return os.cpu_count() or 1
+
+
+def set_oracle_threads(n):
+    """Number of OpenMP threads of the oracle's loops (the OpenMP runtime liborc.so is linked against)."""
+    import ctypes
+    from oracle import orc
+    orc.lib()
+    ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
 
 
 def make_workload(name, n):
@@ -329,31 +346,104 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel class
+    # ---- rooflines.  The fp64 peak is measured in this run (a DFMA loop on every SM for >= 0.5 s, after the timed region).
     peaks, which = measured_peaks()
-    nall = int(np.prod(prim.shape)) // 8
+    psampler = ClockSampler(local)
+    dfma_per_s, peak_ms, nsm = phx.debug_fp64_peak(0.5)
+    pclk = psampler.stop()
+    r64 = dfma_per_s                                   # fp64 thread-instructions per second the pipe issues (any of dadd / dmul / dfma)
+    fp64_peak = {"dfma_per_s": dfma_per_s, "tflops": 2.0 * dfma_per_s / 1e12, "seconds": peak_ms * 1e-3, "sms": nsm,
+                 "sm_mhz_during": pclk["sm_mhz"], "reasons_during": pclk["reasons"],
+                 "nominal_tflops": nsm * 64 * 2 * (peaks.get("sm_max_mhz", 1965.0) * 1e6) / 1e12,
+                 "how": "phx_debug_fp64_peak: 8 independent DFMA chains per thread, 64 warps per SM, CUDA events"}
+    nall = int(np.prod(prim.shape)) // prim.shape[1]
     per_launch_bytes = {k: v * zones for k, v in ALGO_BYTES_PER_ZONE.items()}
     per_launch_bytes["fill_ghosts"] = (nall - zones) * 128.0
     kern = {k: {"ms_total": v[0], "launches": v[1], "ms_per_launch": v[0] / v[1], "share": v[0] / ms}
             for k, v in prof.items() if v[1] > 0}
-    top = max(kern, key=lambda k: kern[k]["ms_total"])
-    dur = kern[top]["ms_per_launch"] * 1e-3
-    hbm = per_launch_bytes[top] / dur / 1e9
-    flops = ALGO_FLOP_PER_ZONE.get(top, 0.0) * zones / dur / 1e12
-    traffic = NCU_TRAFFIC.get(args.n, {}).get(top)
-    if flops / FP64_PEAK_TFLOPS >= hbm / peaks["hbm_gbs"]:
-        roofline = {"kernel": top, "bound": "alu", "achieved": flops, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
-                    "frac": flops / FP64_PEAK_TFLOPS, "traffic": traffic,
-                    "peak_source": "derived: 148 SM x 64 fp64 lanes x 2 x 1.965 GHz (DFMA loop measured %.1f)" % FP64_MEASURED_DFMA_TFLOPS,
-                    "hbm_gbs_achieved": hbm, "hbm_frac": hbm / peaks["hbm_gbs"]}
-    else:
-        roofline = {"kernel": top, "bound": "hbm", "achieved": hbm, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                    "frac": hbm / peaks["hbm_gbs"], "traffic": traffic, "peak_source": which,
-                    "fp64_tflops_achieved": flops, "fp64_frac": flops / FP64_PEAK_TFLOPS}
-    roofline.update(ms_per_launch=kern[top]["ms_per_launch"], share_of_step=kern[top]["share"])
-    # whole-step fp64 fraction: algorithmic flop of all launches of one step / step time
-    step_flop = 2.0 * sum(ALGO_FLOP_PER_ZONE[k] for k in ("sweep_x", "sweep_y", "sweep_z", "update")) + ALGO_FLOP_PER_ZONE["cfl"]
-    roofline["step_fp64_frac"] = step_flop * zones / (ms / K * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+    counts, capture, counts_ok = load_counts()
+    if args.workload != "cfg4" or args.n != 256:
+        counts_ok = False                               # the counts are those of the 256^3 bench workload
+
+    def instr(k):   # executed fp64 thread-instructions / flop per zone and launch of class k (update: both stages averaged)
+        if k == "update":
+            return 0.5 * (counts["update"]["fp64_instr_per_zone"] + counts["update_cfl"]["fp64_instr_per_zone"]), \
+                   0.5 * (counts["update"]["flop_per_zone"] + counts["update_cfl"]["flop_per_zone"])
+        if k in counts:
+            return counts[k]["fp64_instr_per_zone"], counts[k]["flop_per_zone"]
+        return 0.0, 0.0
+
+    def traffic(k):
+        if k == "update":
+            return 0.5 * sum(counts[c]["dram_read_bytes"] + counts[c]["dram_write_bytes"] for c in ("update", "update_cfl"))
+        return counts[k]["dram_read_bytes"] + counts[k]["dram_write_bytes"] if k in counts else None
+
+    roofline = None
+    if all(k in kern for k in SWEEPS + ("update",)):
+        # (1) the dominant kernel CLASS: the three reconstruct + Riemann sweeps (one kernel template, x and marching y / z)
+        sw_ms = sum(kern[k]["ms_total"] for k in SWEEPS)
+        sw_launch = sum(kern[k]["launches"] for k in SWEEPS)
+        sw_dur = sw_ms / sw_launch * 1e-3
+        sw_bytes = sum(per_launch_bytes[k] for k in SWEEPS) / 3.0
+        roofline = {"kernel": "sweeps: k_sweep_x + k_sweep_march<y> + k_sweep_march<z> (fused reconstruct + Riemann + divergence)",
+                    "bound": "alu", "unit": "TFLOP/s", "peak": fp64_peak["tflops"],
+                    "peak_source": "measured in this run (DFMA loop, %.2f s, SM clock %s MHz): 2 flop x %.3e DFMA/s; nominal %d SM x 64 lanes x 2 x %.0f MHz = %.1f"
+                                   % (fp64_peak["seconds"], pclk["sm_mhz"], dfma_per_s, nsm, peaks.get("sm_max_mhz", 1965.0), fp64_peak["nominal_tflops"]),
+                    "ms_per_launch": sw_dur * 1e3, "share_of_step": sw_ms / ms,
+                    "hbm_gbs_achieved": sw_bytes / sw_dur / 1e9, "hbm_frac": sw_bytes / sw_dur / 1e9 / peaks["hbm_gbs"],
+                    "counts_from": f"{COUNTS_FILE} capture {capture}" if counts_ok else None}
+        if counts_ok:
+            ins = sum(instr(k)[0] for k in SWEEPS) / 3.0 * zones
+            flo = sum(instr(k)[1] for k in SWEEPS) / 3.0 * zones
+            roofline.update(achieved=flo / sw_dur / 1e12, frac=flo / sw_dur / 1e12 / fp64_peak["tflops"],
+                            traffic=sum(traffic(k) for k in SWEEPS) / 3.0,
+                            instr_rate={"achieved": ins / sw_dur, "peak": r64, "unit": "fp64 thread-instr/s", "frac": ins / sw_dur / r64})
+        else:
+            roofline.update(achieved=None, frac=None, traffic=None, instr_rate=None,
+                            note="no ncu capture of these kernel sources under profiles/: fp64 figures withheld")
+        # (2) the HBM-bound kernel: flux-CT + update + con2prim + floors
+        up_dur = kern["update"]["ms_per_launch"] * 1e-3
+        up = {"kernel": "k_update (flux-CT + divergence + sources + RK combine + con2prim + floors)", "bound": "hbm", "unit": "GB/s",
+              "peak": peaks["hbm_gbs"], "peak_source": which,
+              "achieved": UPDATE_METHOD_BYTES_PER_ZONE * zones / up_dur / 1e9,
+              "frac": UPDATE_METHOD_BYTES_PER_ZONE * zones / up_dur / 1e9 / peaks["hbm_gbs"],
+              "bytes_per_zone": UPDATE_METHOD_BYTES_PER_ZONE,
+              "design_bytes_per_zone": ALGO_BYTES_PER_ZONE["update"],
+              "design_frac": per_launch_bytes["update"] / up_dur / 1e9 / peaks["hbm_gbs"],
+              "ms_per_launch": up_dur * 1e3, "share_of_step": kern["update"]["share"]}
+        if counts_ok:
+            up.update(traffic=traffic("update"), traffic_over_algorithmic=traffic("update") / (UPDATE_METHOD_BYTES_PER_ZONE * zones),
+                      fp64_instr_rate_frac=instr("update")[0] * zones / up_dur / r64)
+        else:
+            up.update(traffic=None, traffic_over_algorithmic=None)
+        roofline["update"] = up
+        # (3) the step as SURVEY.md 8(d) defines it: T_roof = sum over launches of max(bytes / BW, fp64 instructions / R64)
+        if counts_ok:
+            t_roof, tot_ins, tot_flo = 0.0, 0.0, 0.0
+            for k, v in kern.items():
+                nl = v["launches"] / K
+                by = per_launch_bytes.get(k, 0.0) if k != "update" else UPDATE_METHOD_BYTES_PER_ZONE * zones
+                ik, fk = instr(k)
+                t_roof += nl * max(by / (peaks["hbm_gbs"] * 1e9), ik * zones / r64)
+                tot_ins += nl * ik * zones
+                tot_flo += nl * fk * zones
+            step_s = ms / K * 1e-3
+            roofline["step"] = {"t_roof_ms": t_roof * 1e3, "ms_per_step": ms / K, "frac_of_per_kernel_rooflines": t_roof / step_s,
+                                "fp64_instr_per_zone_cycle": tot_ins / zones, "instr_rate_frac": tot_ins / step_s / r64,
+                                "flop_rate_frac": tot_flo / step_s / (2.0 * r64),
+                                "binding": "fp64 instruction issue (the whole step is ALU-bound: %.0f fp64 instructions per zone-cycle against %.0f algorithmic bytes)"
+                                           % (tot_ins / zones, 2 * (sum(ALGO_BYTES_PER_ZONE[k] for k in SWEEPS) + UPDATE_METHOD_BYTES_PER_ZONE)),
+                                "claim": "north_star's >= 50 % of the binding roofline is claimed on instr_rate_frac: the fp64 pipe issues one "
+                                         "thread-instruction per lane and cycle whether it is an add, a multiply or a fused multiply-add, and "
+                                         "only 47 % of this path's fp64 instructions can be fused; flop_rate_frac counts the same work against "
+                                         "2 flop per lane and cycle"}
+    roofline_out = roofline
+    if roofline_out is not None:
+        if not counts_ok:
+            # without a capture of these sources only the byte-counted roofline can be stated: the update kernel's
+            roofline_out = dict(roofline["update"], sweeps=roofline)
+            del roofline["update"]
+        roofline_out["fp64_peak"] = fp64_peak
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms / K,
@@ -365,16 +455,20 @@ def run_ours(args):
         "e2e": e2e,
         "graph_replay": {"value": value_graph, "unit": UNIT, "ms_per_step": ms_graph / K,
                          "call": "phx_evolve_device(nsteps=K): one RK2 step captured into a CUDA graph and replayed K times"},
-        "gpu_launches": int(launches), "roofline": roofline, "clocks": clocks,
+        "gpu_launches": int(launches), "roofline": roofline_out, "clocks": clocks,
         "kernels": kern, "state_finite": finite, "c2p_failed_cells": bad,
     }
-    if args.workload != "cfg4" or args.n != 256:
-        line["roofline"] = None if args.workload != "cfg4" else roofline
     if not args.no_cpu_baseline and world >= 1:
         ws, steps, what = oracle_sample(args.workload)
         zs, per_step = time_oracle(0, steps, ws)
         line["cpu_baseline"] = {"value": zs * steps / sum(per_step), "unit": UNIT, "cores": oracle_cores(), "kind": "oracle",
                                 "sample": f"{what} ({zs * steps} zone-cycles; {zones * K} timed on the GPU)"}
+        # the same oracle on ONE host thread, on a 64^3 box of the config-4 recipe, one step
+        set_oracle_threads(1)
+        z1, per1 = time_oracle(64, 1)
+        set_oracle_threads(oracle_cores())
+        line["cpu_baseline"]["single_thread"] = {"value": z1 / sum(per1), "unit": UNIT, "cores": 1,
+                                                 "sample": "config-4 recipe at 64^3, one RK2 step + CFL"}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
