@@ -164,10 +164,12 @@ int phx_profile_read(phx_mesh* mesh, double* h_ms, unsigned long long* h_count);
 
 /* Peak of the fp64 pipe, measured: a loop of independent fused multiply-adds (8 chains per thread, 64 warps per SM) on every
  * SM for at least `min_seconds` (0 < min_seconds <= 10) after a calibration launch, timed with CUDA events on `stream`.
- * *h_dfma_per_s (HOST, required) receives DFMA thread-instructions per second (x 2 = flop/s); *h_ms (HOST, nullable) the
- * duration of the timed launch; *h_nsm (HOST, nullable) the SM count of the current device.  Synchronises `stream`.
+ * *h_dfma_per_s (HOST, required) receives DFMA thread-instructions per second (x 2 = flop/s) of that sustained launch;
+ * *h_dfma_per_s_burst (HOST, nullable) the rate of the short calibration launch before it (min_seconds / 20: the burst figure,
+ * before a power cap acts); *h_ms (HOST, nullable) the duration of the timed launch; *h_nsm (HOST, nullable) the SM count of
+ * the current device.  Synchronises `stream`.
  * The denominator of bench.py's ALU roofline (R64 is to be measured, not assumed). */
-int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, double* h_ms, int* h_nsm, void* stream);
+int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, double* h_dfma_per_s_burst, double* h_ms, int* h_nsm, void* stream);
 
 const char* phx_last_error(void);
 

@@ -1194,7 +1194,7 @@ __global__ void __launch_bounds__(256) k_fp64_peak(double* __restrict__ sink, lo
   if (t == 123456.789) sink[0] = t;      // never true: keeps the chains alive
 }
 
-extern "C" int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, double* h_ms, int* h_nsm, void* stream) {
+extern "C" int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, double* h_dfma_per_s_burst, double* h_ms, int* h_nsm, void* stream) {
   if (!(min_seconds > 0.0) || min_seconds > 10.0 || !h_dfma_per_s) return fail(PHX_EINVAL, "phx_debug_fp64_peak: min_seconds in (0, 10] and a result pointer required");
   cudaStream_t st = (cudaStream_t)stream;
   int dev = 0, nsm = 0;
@@ -1217,6 +1217,7 @@ extern "C" int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, dou
     if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
     if (pass == 2 || e != cudaSuccess) break;
     const double rate = per_iter * (double)iters / (ms * 1e-3);
+    if (pass == 1 && h_dfma_per_s_burst) *h_dfma_per_s_burst = rate;   // the short second launch: before any power cap acts
     iters = (long long)(min_seconds * rate / per_iter * (pass == 0 ? 0.05 : 1.0)) + 1;
   }
   cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);

@@ -100,7 +100,7 @@ def lib():
         L.phx_launch_count.argtypes = [vp]; L.phx_launch_count.restype = C.c_ulonglong
         L.phx_profile_enable.argtypes = [vp, C.c_int]
         L.phx_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
-        L.phx_debug_fp64_peak.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int), vp]
+        L.phx_debug_fp64_peak.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int), vp]
         L.phx_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -260,7 +260,8 @@ def evolve_host(mesh, h_prim_in, nsteps, cfl, h_prim_out, h_cons_out=None, h_mas
 
 
 def debug_fp64_peak(min_seconds=0.5, stream=None):
-    """Measured peak of the fp64 pipe: (DFMA thread-instructions per second, milliseconds of the timed launch, SM count)."""
-    r, ms, nsm = C.c_double(), C.c_double(), C.c_int()
-    _check(lib().phx_debug_fp64_peak(float(min_seconds), C.byref(r), C.byref(ms), C.byref(nsm), _stream(stream)))
-    return r.value, ms.value, nsm.value
+    """Measured peak of the fp64 pipe: (DFMA thread-instructions per second sustained over min_seconds, the same for the short
+    calibration launch before it, milliseconds of the timed launch, SM count)."""
+    r, rb, ms, nsm = C.c_double(), C.c_double(), C.c_double(), C.c_int()
+    _check(lib().phx_debug_fp64_peak(float(min_seconds), C.byref(r), C.byref(rb), C.byref(ms), C.byref(nsm), _stream(stream)))
+    return r.value, rb.value, ms.value, nsm.value
