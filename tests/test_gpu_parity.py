@@ -131,9 +131,12 @@ def test_cons_to_prim_floors_and_failure_masks():
     got = interior(p, prim_g.cpu().numpy()); ref = interior(p, prim_ref)
     # point-wise relative comparison (states span many decades)
     den = np.maximum(np.abs(ref), 1e-3 * np.abs(ref).max(axis=0, keepdims=True) + 1e-300)
-    # 1e-8: the inversion's condition number on these extreme states (W up to ~16, eps down to 1e-4, b^2/rho >> 1)
-    # is ~1e7-1e8 ulp (2e-9 seen for bisection-vs-exact on such states); config-like states are held
-    # to 1e-12 by test_cons_to_prim_matches_oracle
+    # 1e-8: the inversion's condition number on these extreme states (W up to ~16, eps down to 1e-4, b^2/rho up to 2e5).
+    # Measured against a 50-digit inversion of the same conserved doubles (tests/test_c2p_accuracy.py and a one-off run over
+    # all 4096 states of this test): on the magnetically dominated cells (b^2/rho > 1e4) BOTH sides are 1e-10 ... 3e-9 away
+    # from the exact inverse; the largest difference between them, 2.4e-9 in one cell with b^2/rho = 1.4e5, is 2.8e-9 of the
+    # CUDA path's secant and 3.9e-10 of the oracle's bisection.  Config-like states are held to 1e-12 by
+    # test_cons_to_prim_matches_oracle.
     print("floors / failure masks: max point-wise relative difference of the primitives", (np.abs(got - ref) / den).max())
     assert (np.abs(got - ref) / den).max() < 1e-8
     cg = interior(p, cons.cpu().numpy()); cr = interior(p, cons_ref)
