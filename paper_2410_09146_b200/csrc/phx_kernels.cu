@@ -10,12 +10,14 @@
 //   k_update       flux-CT + accumulated divergence + geometric sources + RK combine + con2prim + floors, one thread per cell
 //   k_fill_ghosts  periodic / outflow / block-to-block ghost copies in one gather pass over the ghost cells
 // and k_cfl_partial / k_cfl_final (warp-shuffle min reduction), k_cfl_final_slots (fused into stage 2), k_prim_to_cons,
-// k_c2p, k_excision_flags; phx_evolve_device replays one captured step as a CUDA graph.
+// k_c2p, k_excision_flags, k_fp64_peak (the measured denominator of the ALU roofline); phx_evolve_device replays one captured
+// step as a CUDA graph, or runs a small 1-D mesh entirely inside one thread block (k_evolve_1d).
 #include "phx_device.cuh"
 #include "../../include/phx.h"
 
 #include <new>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 using namespace phx;
@@ -747,6 +749,7 @@ struct phx_mesh {
   double* flux[3];
   double* racc;               // divergence of the non-magnetic flux components accumulated by the sweeps: [block][5+nscalar][cells]
   int store_all_fluxes;       // phx_debug_enable_flux: the sweeps also store the non-magnetic flux components
+  int small_1d;               // phx_evolve_device may take the one-block path for small 1-D meshes (PHX_SMALL_1D=0 switches it off)
   unsigned char* xfl;
   double* partial;
   int npartial;
@@ -851,6 +854,7 @@ extern "C" int phx_init_mesh(const phx_params* p, void* stream, phx_mesh** out) 
   m.nvar = NV + p->nscalar;
   m.xs_min = p->scalar_min; m.xs_max = p->scalar_max;
   m.floor_form = p->floor_form; m.fl_arho = p->floor_alpha_rho; m.fl_aeps = p->floor_alpha_eps;
+  { const char* e = getenv("PHX_SMALL_1D"); M->small_1d = e ? atoi(e) != 0 : 1; }
   M->nall = (long long)m.nblk * m.ncell;
   M->ninterior = (long long)m.nblk * m.n[0] * m.n[1] * m.n[2];
   if (M->nall * m.nvar >= (1LL << 40)) { delete M; return fail(PHX_EINVAL, "phx_init_mesh: field too large"); }
@@ -1228,6 +1232,151 @@ extern "C" int phx_debug_fp64_peak(double min_seconds, double* h_dfma_per_s, dou
   return PHX_OK;
 }
 
+// ---- small one-dimensional meshes: the whole run in ONE thread block ---------------------------------------------------
+// A 1-D mesh of a few hundred zones (BASELINE.json config 1: 256 zones) is pure launch latency on the general path: 8 kernels
+// of 2-3 us per step.  Here one thread block owns the mesh (one thread per cell, the two ghost-adjacent cells included) and
+// loops over `nsteps` RK2 steps on the device: per stage reconstruct + Riemann flux with the face states and fluxes exchanged
+// through shared memory, divergence, RK combination, con2prim + floors, ghost cells, and after the second stage the block-wide
+// maximum of the signal speeds gives the next time step.  Barriers are __syncthreads; nothing leaves the SM between stages
+// but the few KB of state in L1 / L2.  Same device functions and the same expressions as k_sweep_x / update_cell (flat
+// metric, no passive scalar, constant floors, no excision): the results are the bits of the general path.
+constexpr int SM1_MAXT = 512;
+template <int RECON>
+__global__ void __launch_bounds__(SM1_MAXT, 1) k_evolve_1d(MeshDev m, int nsteps, double cfl, double* __restrict__ d_dt, double* __restrict__ d_t,
+                                                          double* __restrict__ cons0, double* __restrict__ cons, double* __restrict__ prim,
+                                                          unsigned char* __restrict__ mask) {
+  constexpr int HW = ReconTraits<RECON>::HW;
+  extern __shared__ double smem1[];
+  const int T = blockDim.x;
+  double (*sh)[SM1_MAXT] = reinterpret_cast<double (*)[SM1_MAXT]>(smem1);                  // upper-face states, NV rows
+  double (*shF)[SM1_MAXT] = reinterpret_cast<double (*)[SM1_MAXT]>(smem1 + NV * SM1_MAXT);   // face fluxes, NV rows
+  __shared__ double red[SM1_MAXT / 32];
+  __shared__ double dt_sh;
+  const int t = threadIdx.x;
+  const int n = m.n[0], g = m.g[0];
+  const bool valid = t < n + 2;                    // cell i = g - 1 + t
+  const int i = g - 1 + t;
+  const bool interior = t >= 1 && t <= n;
+  (void)T;
+  for (int step = 0; step < nsteps; ++step) {
+    if (t == 0) { dt_sh = *d_dt; if (d_t) *d_t += dt_sh; }
+    __syncthreads();
+    const double dt = dt_sh;
+    double speed = 0.0;
+    for (int stage = 0; stage < 2; ++stage) {
+      // stage 1: U~1 = U~0 + dt R -> cons0 (scratch); stage 2: U~ = (U~0 + U~1)/2 + dt/2 R -> cons   (phx_rk2_step)
+      const double g0 = stage == 0 ? 1.0 : 0.5, g1 = stage == 0 ? 0.0 : 0.5;
+      const double bdt = (stage == 0 ? 1.0 : 0.5) * dt;
+      const double* c0 = cons;
+      const double* cin = stage == 0 ? cons : cons0;
+      double* cout = stage == 0 ? cons0 : cons;
+      double qm[NV], qp[NV], F[NV];
+      if (valid) {
+        double centre[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          double f[2 * HW + 1];
+#pragma unroll
+          for (int s = 0; s <= 2 * HW; ++s) f[s] = prim[v * m.ncell + i + (s - HW)];
+          centre[v] = f[HW];
+          recon1<RECON>(f, qm[v], qp[v]);
+        }
+        positivity_fallback<0, RECON, 0>(m, 0.0, 0.0, 0.0, centre, qm, qp);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) sh[v][t] = qp[v];
+      }
+      __syncthreads();
+      const bool face = valid && t > 0;            // face (i - 1/2)
+      if (face) {
+        double qL[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) qL[v] = sh[v][t - 1];
+        Geo<0> G;
+        face_flux<0, 0, 0>(m, G, qL, qm, F);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) shF[v][t] = F[v];
+      }
+      __syncthreads();
+      if (interior) {
+        double R[NV], U[NV], q[NV];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) R[v] = 0.0 - (shF[v][t + 1] - F[v]) * m.rdx[0];
+        R[BX] = 0.0;                               // F~^x[B^x] = 0: the update leaves B^x alone in 1-D
+        q[RHO] = prim[RHO * m.ncell + i];
+        q[UX] = prim[UX * m.ncell + i]; q[UY] = prim[UY * m.ncell + i]; q[UZ] = prim[UZ * m.ncell + i];
+        q[UU] = prim[UU * m.ncell + i];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const long long id = v * m.ncell + i;
+          U[v] = (g1 != 0.0) ? g0 * c0[id] + g1 * cin[id] + bdt * R[v] : g0 * c0[id] + bdt * R[v];
+        }
+        Geo<0> G;
+        const double mu_guess = c2p_guess<0>(G, q, m.gam);
+        unsigned mk = c2p_cell<0>(m, G, m.rho_floor, m.eps_floor, U, q, mu_guess);
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+          const long long id = v * m.ncell + i;
+          cout[id] = U[v];
+          prim[id] = q[v];
+        }
+        mask[i] = (unsigned char)mk;
+        if (stage == 1) {
+          double lam[3];
+          max_speeds<0>(q, G, m.gam, lam);
+          speed = cfl_guard(lam[0] * m.rdx[0]);
+        }
+      }
+      __syncthreads();
+      // ghost cells: periodic wrap or zero-gradient copy (k_fill_ghosts in one dimension)
+      if (t < 2 * g) {
+        const int l = t < g ? t : t + n;           // allocated index of the ghost cell
+        int li = l - g;
+        if (li < 0) li = (m.bc[0][0] == 0) ? li + n : 0;
+        else li = (m.bc[0][1] == 0) ? li - n : n - 1;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) prim[v * m.ncell + l] = prim[v * m.ncell + li + g];
+      }
+      __syncthreads();
+    }
+    // next time step: cfl / max over the cells of |lambda|/dx
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) speed = fmax(speed, __shfl_xor_sync(0xffffffffu, speed, o));
+    if ((t & 31) == 0) red[t >> 5] = speed;
+    __syncthreads();
+    if (t == 0) {
+      double v = red[0];
+      for (int w = 1; w < (blockDim.x + 31) / 32; ++w) v = fmax(v, red[w]);
+      *d_dt = cfl_dt_of(cfl, v);
+    }
+    __syncthreads();
+  }
+}
+
+// the single-block path applies to: one block, x the only active direction, flat metric without shift, no passive scalar,
+// constant floors, a mesh that fits one thread block
+static bool small_1d_eligible(const phx_mesh* M) {
+  const MeshDev& m = M->m;
+  return m.nblk == 1 && m.act[0] && !m.act[1] && !m.act[2] && m.metric == 0 && m.nvar == NV && m.floor_form == 0 && !m.excise &&
+         m.n[0] + 2 <= SM1_MAXT && !M->store_all_fluxes && M->small_1d;
+}
+
+static int launch_evolve_1d(phx_mesh* M, int nsteps, double cfl, double* d_dt, double* d_t, double* d_cons0, double* d_cons, double* d_prim,
+                            unsigned char* d_mask, cudaStream_t st) {
+  const MeshDev& m = M->m;
+  const int threads = ((m.n[0] + 2 + 31) / 32) * 32;
+  const size_t smem = 2 * NV * SM1_MAXT * sizeof(double);
+#define EV1(REC) case REC: { static bool once = false; \
+    if (!once) { CUDA_TRY(cudaFuncSetAttribute(k_evolve_1d<REC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "cudaFuncSetAttribute"); once = true; } \
+    k_evolve_1d<REC><<<1, threads, smem, st>>>(m, nsteps, cfl, d_dt, d_t, d_cons0, d_cons, d_prim, d_mask); } break;
+  switch (m.recon) {
+    EV1(0) EV1(1) EV1(2) EV1(3) EV1(4) EV1(5)
+    default: return fail(PHX_EUNSUPPORTED, "k_evolve_1d: unknown reconstruction");
+  }
+#undef EV1
+  LAUNCH_CHECK(M, "k_evolve_1d");
+  return PHX_OK;
+}
+
 // ---- host-buffer path ------------------------------------------------------------------------------------------
 __global__ void k_accumulate_time(double* __restrict__ t, const double* __restrict__ dt) { *t += *dt; }
 
@@ -1247,6 +1396,8 @@ extern "C" int phx_evolve_device(phx_mesh* M, int nsteps, double cfl, double* d_
     return fail(PHX_EINVAL, "phx_evolve_device: null, misaligned or aliased argument, nsteps < 0 or cfl <= 0");
   cudaStream_t st = (cudaStream_t)stream;
   if (nsteps == 0) return PHX_OK;
+  // a small 1-D mesh runs all its steps in one launch of one thread block (no per-kernel timing there: one kernel)
+  if (!M->ev && small_1d_eligible(M)) return launch_evolve_1d(M, nsteps, cfl, d_dt, d_t, d_cons0, d_cons, d_prim, d_mask, st);
   // per-kernel timing records events around every launch, which a replayed graph cannot serve: launch directly then
   if (M->ev || nsteps < 2) {
     for (int s = 0; s < nsteps; ++s) {
