@@ -594,42 +594,16 @@ __global__ void __launch_bounds__(256) k_prim_to_cons(MeshDev m, const double* _
 }
 
 // ---- ghost fill: one gather pass -------------------------------------------------------------------
-// blockIdx.z = block; the threads enumerate the ghost cells of the block only: first the 2 g_z full k-planes, then the
-// 2 g_y full rows of every interior k-plane, then the 2 g_x end cells of every interior row (nA, nB: sizes of the first
-// two groups, ntot: all ghost cells of one block).
-__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, int nA, int nB, int ntot) {
-  int t = blockIdx.x * 256 + threadIdx.x;
-  if (t >= ntot) return;
-  int l[3];
-  if (t < nA) {
-    const int plane = m.na[0] * m.na[1];
-    const int kz = t / plane;
-    t -= kz * plane;
-    l[2] = kz < m.g[2] ? kz : kz + m.n[2];
-    l[1] = t / m.na[0];
-    l[0] = t - l[1] * m.na[0];
-  } else if (t < nA + nB) {
-    t -= nA;
-    const int per = 2 * m.g[1] * m.na[0];
-    const int kk = t / per;
-    t -= kk * per;
-    const int jy = t / m.na[0];
-    l[2] = m.g[2] + kk;
-    l[1] = jy < m.g[1] ? jy : jy + m.n[1];
-    l[0] = t - jy * m.na[0];
-  } else {
-    t -= nA + nB;
-    const int w = 2 * m.g[0];
-    const int row = t / w;
-    const int ix = t - row * w;
-    const int kk = row / m.n[1];
-    l[2] = m.g[2] + kk;
-    l[1] = m.g[1] + (row - kk * m.n[1]);
-    l[0] = ix < m.g[0] ? ix : ix + m.n[0];
-  }
-  const int b = blockIdx.z;
-  int cb[3], sb[3], sl[3];
-  block_coords(m, b, cb);
+// blockIdx.z = block; the threads enumerate the ghost cells of the block only: first the k-planes below and above the
+// interior, then the rows below and above the interior rows of every interior k-plane, then the end cells of every interior
+// row (nA, nB: sizes of the first two groups, ntot: all ghost cells enumerated).
+// GhostShell: the ghost cells within dep[d] <= g[d] layers of the interior (the whole frame: dep = g).  The first stage of a
+// fused two-stage step fills only the layers its second stage reads: stencil half-width + 1 along a sweep, 1 across it.
+struct GhostShell { int dep[3]; int nA, nB, ntot; };
+
+// source of the ghost cell l (allocated indices) of the block at coordinates cb: element index of its variable 0
+__device__ __forceinline__ long long ghost_source(const MeshDev& m, const int* cb, const int* l) {
+  int sb[3], sl[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
     // source cell in block-local terms: inside this block, in the neighbour block, wrapped or clamped at a domain face
@@ -648,15 +622,76 @@ __global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restri
     sl[d] = li + m.g[d];
   }
   const int bs = (sb[2] * m.nb[1] + sb[1]) * m.nb[0] + sb[0];
-  const long long src = (long long)bs * m.nvar * m.ncell + (long long)sl[2] * m.sk + (long long)sl[1] * m.sj + sl[0];
+  return (long long)bs * m.nvar * m.ncell + (long long)sl[2] * m.sk + (long long)sl[1] * m.sj + sl[0];
+}
+
+// VEC = 2: one thread copies two x-adjacent ghost cells (n_x, g_x and the x depth of the shell even: every run of ghost cells
+// along x then starts at an even, 16-byte aligned index) with one 16-byte load and store per variable where the two sources
+// are adjacent too (everywhere but at an outflow face, whose ghosts all copy the same cell).
+template <int VEC>
+__global__ void __launch_bounds__(256) k_fill_ghosts(MeshDev m, double* __restrict__ prim, GhostShell gs) {
+  int t = blockIdx.x * 256 + threadIdx.x;
+  if (t >= gs.ntot) return;
+  int l[3];
+  const int w0 = (m.n[0] + 2 * gs.dep[0]) / VEC, w1 = m.n[1] + 2 * gs.dep[1];     // extent of the shell's bounding box (x in units of VEC cells)
+  const int o0 = m.g[0] - gs.dep[0], o1 = m.g[1] - gs.dep[1], o2 = m.g[2] - gs.dep[2];
+  if (t < gs.nA) {                      // the k-planes below and above the interior
+    const int plane = w0 * w1;
+    const int kz = t / plane;
+    t -= kz * plane;
+    l[2] = kz < gs.dep[2] ? o2 + kz : m.g[2] + m.n[2] + (kz - gs.dep[2]);
+    const int jy = t / w0;
+    l[1] = o1 + jy;
+    l[0] = o0 + VEC * (t - jy * w0);
+  } else if (t < gs.nA + gs.nB) {       // the rows below and above the interior rows of every interior k-plane
+    t -= gs.nA;
+    const int per = 2 * gs.dep[1] * w0;
+    const int kk = t / per;
+    t -= kk * per;
+    const int jy = t / w0;
+    l[2] = m.g[2] + kk;
+    l[1] = jy < gs.dep[1] ? o1 + jy : m.g[1] + m.n[1] + (jy - gs.dep[1]);
+    l[0] = o0 + VEC * (t - jy * w0);
+  } else {                              // the end cells of every interior row
+    t -= gs.nA + gs.nB;
+    const int w = 2 * gs.dep[0] / VEC;
+    const int row = t / w;
+    const int ix = VEC * (t - row * w);
+    const int kk = row / m.n[1];
+    l[2] = m.g[2] + kk;
+    l[1] = m.g[1] + (row - kk * m.n[1]);
+    l[0] = ix < gs.dep[0] ? o0 + ix : m.g[0] + m.n[0] + (ix - gs.dep[0]);
+  }
+  const int b = blockIdx.z;
+  int cb[3];
+  block_coords(m, b, cb);
+  const long long src = ghost_source(m, cb, l);
   const long long dst = (long long)b * m.nvar * m.ncell + (long long)l[2] * m.sk + (long long)l[1] * m.sj + l[0];
-  double v[NV + 1];
+  if constexpr (VEC == 1) {
+    double v[NV + 1];
 #pragma unroll
-  for (int q = 0; q < NV; ++q) v[q] = prim[src + q * m.ncell];
-  if (m.nvar > NV) v[XS] = prim[src + XS * m.ncell];
+    for (int q = 0; q < NV; ++q) v[q] = prim[src + q * m.ncell];
+    if (m.nvar > NV) v[XS] = prim[src + XS * m.ncell];
 #pragma unroll
-  for (int q = 0; q < NV; ++q) prim[dst + q * m.ncell] = v[q];
-  if (m.nvar > NV) prim[dst + XS * m.ncell] = v[XS];
+    for (int q = 0; q < NV; ++q) prim[dst + q * m.ncell] = v[q];
+    if (m.nvar > NV) prim[dst + XS * m.ncell] = v[XS];
+  } else {
+    int l1[3] = {l[0] + 1, l[1], l[2]};
+    const long long src1 = ghost_source(m, cb, l1);
+    double2 v[NV + 1];
+    if (src1 == src + 1 && (src & 1) == 0) {
+#pragma unroll
+      for (int q = 0; q < NV; ++q) v[q] = *reinterpret_cast<const double2*>(prim + src + q * m.ncell);
+      if (m.nvar > NV) v[XS] = *reinterpret_cast<const double2*>(prim + src + XS * m.ncell);
+    } else {
+#pragma unroll
+      for (int q = 0; q < NV; ++q) { v[q].x = prim[src + q * m.ncell]; v[q].y = prim[src1 + q * m.ncell]; }
+      if (m.nvar > NV) { v[XS].x = prim[src + XS * m.ncell]; v[XS].y = prim[src1 + XS * m.ncell]; }
+    }
+#pragma unroll
+    for (int q = 0; q < NV; ++q) *reinterpret_cast<double2*>(prim + dst + q * m.ncell) = v[q];
+    if (m.nvar > NV) *reinterpret_cast<double2*>(prim + dst + XS * m.ncell) = v[XS];
+  }
 }
 
 // ---- CFL: warp-shuffle min reduction ------------------------------------------------------------------
@@ -937,9 +972,9 @@ extern "C" int phx_debug_flux(const phx_mesh* M, int d, double* d_out, void* str
   return PHX_OK;
 }
 
-// PHX_BUILD_SUBSET (development only): instantiate the flat-metric WENO5-Z / PLM kernels alone, for quick A/B builds
+// PHX_BUILD_SUBSET (development only): instantiate the flat-metric WENO5-Z / PLM and the Kerr-Schild PLM kernels alone, for quick A/B builds
 #ifdef PHX_BUILD_SUBSET
-#define DISPATCH_METRIC(mesh, CALL) do { CALL(0); } while (0)
+#define DISPATCH_METRIC(mesh, CALL) do { if ((mesh)->m.metric == 1) { CALL(1); } else { CALL(0); } } while (0)
 #else
 #define DISPATCH_METRIC(mesh, CALL)                 \
   do {                                              \
@@ -963,16 +998,29 @@ extern "C" int phx_prim_to_cons(const phx_mesh* M, const double* d_prim, double*
   return PHX_OK;
 }
 
-extern "C" int phx_fill_ghosts(const phx_mesh* M, double* d_prim, void* stream) {
-  if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
+// depth < 0: the whole frame; otherwise the layers a stage of this mesh's reconstruction reads (half-width + 1, at most g)
+static int fill_ghosts_impl(const phx_mesh* M, double* d_prim, int depth, cudaStream_t st) {
   if (M->nall == M->ninterior) return PHX_OK;
-  { ProfScope ps(M, PHX_K_FILL_GHOSTS, (cudaStream_t)stream);
+  { ProfScope ps(M, PHX_K_FILL_GHOSTS, st);
     const MeshDev& m = M->m;
-    const long long nA = 2LL * m.g[2] * m.na[1] * m.na[0], nB = 2LL * m.n[2] * m.g[1] * m.na[0], nC = 2LL * m.n[2] * m.n[1] * m.g[0];
+    GhostShell gs;
+    for (int d = 0; d < 3; ++d) gs.dep[d] = (depth < 0 || depth > m.g[d]) ? m.g[d] : depth;
+    gs.dep[0] = m.g[0];      // along x always the whole depth: a thinner shell would write partial 32-byte sectors (measured: no gain)
+    // two cells per thread where every run of ghost cells along x is even and 16-byte aligned (field strides: ncell, sk, sj even)
+    const int vec = (m.act[0] && m.n[0] % 2 == 0 && m.g[0] % 2 == 0 && gs.dep[0] % 2 == 0) ? 2 : 1;
+    const long long w0 = (m.n[0] + 2 * gs.dep[0]) / vec, w1 = m.n[1] + 2 * gs.dep[1];
+    const long long nA = 2LL * gs.dep[2] * w1 * w0, nB = 2LL * m.n[2] * gs.dep[1] * w0, nC = 2LL * m.n[2] * m.n[1] * gs.dep[0] / vec;
+    gs.nA = (int)nA; gs.nB = (int)nB; gs.ntot = (int)(nA + nB + nC);
     const dim3 grid((unsigned)((nA + nB + nC + 255) / 256), 1, m.nblk);
-    k_fill_ghosts<<<grid, 256, 0, (cudaStream_t)stream>>>(m, d_prim, (int)nA, (int)nB, (int)(nA + nB + nC)); }
+    if (vec == 2) k_fill_ghosts<2><<<grid, 256, 0, st>>>(m, d_prim, gs);
+    else k_fill_ghosts<1><<<grid, 256, 0, st>>>(m, d_prim, gs); }
   LAUNCH_CHECK(M, "k_fill_ghosts");
   return PHX_OK;
+}
+
+extern "C" int phx_fill_ghosts(const phx_mesh* M, double* d_prim, void* stream) {
+  if (!M || !aligned16(d_prim)) return fail(PHX_EINVAL, "phx_fill_ghosts: null or misaligned argument");
+  return fill_ghosts_impl(M, d_prim, -1, (cudaStream_t)stream);
 }
 
 extern "C" int phx_cons_to_prim(const phx_mesh* M, double* d_cons, double* d_prim, unsigned char* d_mask, void* stream) {
@@ -1055,7 +1103,7 @@ static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
   switch (key) {
 #define PHX_CASE(MET, REC) case MET * 6 + REC: if (M->m.nvar == NV) launch_sweeps_t<MET, REC, 0>(M, prim, st); else launch_sweeps_t<MET, REC, 1>(M, prim, st); break;
 #ifdef PHX_BUILD_SUBSET
-    PHX_CASE(0, 1) PHX_CASE(0, 3)
+    PHX_CASE(0, 1) PHX_CASE(0, 3) PHX_CASE(1, 1)
 #else
     PHX_CASE(0, 0) PHX_CASE(0, 1) PHX_CASE(0, 2) PHX_CASE(0, 3) PHX_CASE(0, 4) PHX_CASE(0, 5)
     PHX_CASE(1, 0) PHX_CASE(1, 1) PHX_CASE(1, 2) PHX_CASE(1, 3) PHX_CASE(1, 4) PHX_CASE(1, 5)
@@ -1068,7 +1116,7 @@ static void launch_sweeps(phx_mesh* M, const double* prim, cudaStream_t st) {
 
 static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const double* d_dt, double beta, const double* d_cons0,
                       const double* d_cons_in, double* d_cons_out, double* d_prim, unsigned char* d_mask, cudaStream_t st,
-                      bool reduce_cfl = false) {
+                      bool reduce_cfl = false, bool inner_stage = false) {
   launch_sweeps(M, d_prim, st);
   { cudaError_t e = cudaGetLastError(); if (e != cudaSuccess) return cuda_fail(e, "flux sweep"); }
   FluxPtrs fl;
@@ -1090,7 +1138,10 @@ static int stage_impl(phx_mesh* M, double g0, double g1, double bdt_host, const 
 #undef UPD
   }
   LAUNCH_CHECK(M, "k_update");
-  return phx_fill_ghosts(M, d_prim, st);
+  // a stage whose primitives only the next stage of the same call reads fills the ghost layers that stage's sweeps touch
+  // (stencil half-width + 1); the last stage of a call leaves the whole frame filled, as the header promises
+  const int hw = (M->m.recon == 0) ? 0 : (M->m.recon >= 3 ? 2 : 1);
+  return fill_ghosts_impl(M, d_prim, inner_stage ? hw + 1 : -1, st);
 }
 
 extern "C" int phx_rk_stage(phx_mesh* M, double g0, double g1, double beta_dt, const double* d_cons0, double* d_cons, double* d_prim,
@@ -1106,7 +1157,7 @@ extern "C" int phx_rk2_step(phx_mesh* M, const double* d_dt, double* d_cons0, do
     return fail(PHX_EINVAL, "phx_rk2_step: null, misaligned or aliased argument");
   cudaStream_t st = (cudaStream_t)stream;
   // no copy of U~0: stage 1 reads U~0 = d_cons and writes U~1 into the scratch field; stage 2 combines both into d_cons
-  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st);
+  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st, false, true);
   if (rc != PHX_OK) return rc;
   return stage_impl(M, 0.5, 0.5, 0.0, d_dt, 0.5, d_cons, d_cons0, d_cons, d_prim, d_mask, st);
 }
@@ -1116,7 +1167,7 @@ extern "C" int phx_rk2_step_cfl(phx_mesh* M, double cfl, double* d_dt, double* d
   if (!M || !d_dt || !(cfl > 0.0) || !aligned16(d_cons0) || !aligned16(d_cons) || !aligned16(d_prim) || !d_mask || d_cons0 == d_cons)
     return fail(PHX_EINVAL, "phx_rk2_step_cfl: null, misaligned or aliased argument, or cfl <= 0");
   cudaStream_t st = (cudaStream_t)stream;
-  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st);
+  int rc = stage_impl(M, 1.0, 0.0, 0.0, d_dt, 1.0, d_cons, d_cons, d_cons0, d_prim, d_mask, st, false, true);
   if (rc != PHX_OK) return rc;
   // stage 2 also reduces max sum_d |lambda^d|/dx_d of the new primitives; the final kernel overwrites *d_dt after every
   // block of stage 2 has read it (stream order)

@@ -31,6 +31,9 @@ def small_workloads():
     out["cfg4_turb_24_weno"] = wl.turbulence_box(24)
     out["cfg5_blocks_2x2x2_of_12"] = wl.packed_blocks((2, 2, 2), 12)
     out["cfg5_blocks_3x2x1_of_8"] = wl.packed_blocks((3, 2, 1), 8)
+    # packed blocks with a fifth-order stencil: the first stage of a fused step fills a ghost shell of depth 3, not the frame
+    wb = wl.packed_blocks((2, 2, 2), 12)
+    out["cfg5_blocks_2x2x2_of_12_weno"] = dict(wb, params=dict(wb["params"], recon=wl.RECON_WENO5Z))
     # the paper's WENO5-Z-AOAH (App.B B16-B18) on smooth turbulence and on the shock tube
     out["next1_turb_24_aoah"] = wl.turbulence_box(24, recon=wl.RECON_WENO5Z_AOAH)
     out["next1_shock_tube_200_aoah"] = wl.shock_tube(200, recon=wl.RECON_WENO5Z_AOAH, ng=3)
@@ -282,10 +285,15 @@ def test_many_steps_match_oracle(name, nsteps):
     print(name, nsteps, "steps, err", err)
 
 
-def test_device_dt_step_equals_host_dt_step():
+@pytest.mark.parametrize("name", ["cfg4_turb_24_weno", "cfg5_blocks_2x2x2_of_12", "cfg5_blocks_2x2x2_of_12_weno", "cfg5_blocks_3x2x1_of_8",
+                                  "cfg3_ks_torus_28", "next1_ks_torus_20_aoah", "cfg1_shock_tube_256", "cfg2_box_12_const_llf",
+                                  "next1b_shock_tube_200_mp5"])
+def test_device_dt_step_equals_host_dt_step(name):
     """phx_cfl_dt + phx_rk2_step (dt on the device, the configuration bench.py times) gives bitwise the same
-    state as two phx_rk_stage calls with the same dt passed from the host."""
-    w = WORKLOADS["cfg4_turb_24_weno"]
+    state as two phx_rk_stage calls with the same dt passed from the host.  The fused step fills after its first stage only
+    the ghost layers its second stage reads (stencil half-width + 1 in y and z); every phx_rk_stage call fills the whole frame:
+    equal bits, ghost zones included, on periodic, outflow and block-to-block boundaries and for every stencil width."""
+    w = WORKLOADS[name]
     p = w["params"]
     a = GpuRun(p, w["prim"]); b = GpuRun(p, w["prim"])
     for _ in range(3):
@@ -296,7 +304,8 @@ def test_device_dt_step_equals_host_dt_step():
     assert np.array_equal(ca, cb) and np.array_equal(pa, pb) and np.array_equal(ma, mb)
 
 
-@pytest.mark.parametrize("name", ["cfg4_turb_24_weno", "cfg5_blocks_2x2x2_of_12", "cfg1_shock_tube_256", "cfg3_ks_torus_28"])
+@pytest.mark.parametrize("name", ["cfg4_turb_24_weno", "cfg5_blocks_2x2x2_of_12", "cfg1_shock_tube_256", "cfg3_ks_torus_28",
+                                  "cfg5_blocks_2x2x2_of_12_weno", "next1_ks_torus_20_aoah", "cfg2_box_12_const_llf", "cfg5_blocks_3x2x1_of_8"])
 def test_fused_cfl_step_equals_separate_calls(name):
     """phx_rk2_step_cfl (what bench.py times) = phx_rk2_step followed by phx_cfl_dt, bit for bit, state and time step;
     the time step also matches the oracle's CFL time step of the oracle's new state."""
