@@ -25,7 +25,10 @@
 // second order, bounds; P17 floor forms of PAPER.md:288 against the closed-form Kerr-Schild radius on the axis, in the
 // equatorial plane and for a = 0.  P18 (tests/test_oracle_pins_positivity.py): the positivity fallback of the fifth-order
 // reconstructions in block_fluxes (which cell, which direction, all variables, threshold just below the floors at the cell centre,
-// never for piecewise-linear schemes) on hand-worked stencils.
+// never for piecewise-linear schemes) on hand-worked stencils.  P9 / P15 cover the four linear-wave families of PAPER.md:441
+// (tests/test_oracle_pins_waves.py: eigenmodes against a numerical flux Jacobian of Eq.2-3 written in the test); P19: a
+// finite-amplitude entropy wave, an exact nonlinear solution, is carried at alpha v - beta at second order; con2prim against a
+// 50-digit inversion (tests/test_c2p_accuracy.py).
 //
 // Layout of every field: [block][var][k][j][i], i fastest; var order of primitives
 // P=(rho, W v^1, W v^2, W v^3, rho*eps, B^1, B^2, B^3) (Eq.13) and conserved, stored densitised,
