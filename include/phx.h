@@ -111,7 +111,8 @@ int phx_cfl_dt(const phx_mesh* mesh, const double* d_prim, double cfl, double* d
 
 /* One full RK2 step with the time step read from the device scalar d_dt (no host round trip); the result equals two
  * phx_rk_stage calls bit for bit.  d_cons0 is scratch (same size as d_cons, must not alias it): stage 1 writes its
- * state U~1 there, stage 2 combines U~0 = d_cons and U~1 into d_cons; on return d_cons0 holds U~1. */
+ * state U~1 there, stage 2 combines U~0 = d_cons and U~1 into d_cons; on return d_cons0 holds U~1.  Between the two stages only
+ * the ghost layers stage 2 reads are filled (stencil half-width + 1 in y and z); on return the whole ghost frame of d_prim is. */
 int phx_rk2_step(phx_mesh* mesh, const double* d_dt, double* d_cons0, double* d_cons, double* d_prim,
                  unsigned char* d_mask, void* stream);
 
