@@ -307,7 +307,7 @@ def run_ours(args):
     launches = mesh.launch_count() - l0
     prof = mesh.profile_read()
     mesh.profile_enable(0)
-    bad = int(mask.to(torch.int32).bitwise_and(16 | 32).count_nonzero().item())   # no-convergence / bad-input cells
+    bad = phx.count_masked(mesh, mask, phx.M_NOCONV | phx.M_BAD_INPUT)             # con2prim failures of the last stage
     finite = bool(torch.isfinite(cons).all().item())
     ms, value = aggregate(ms, zones, K, world, "cuda")
 

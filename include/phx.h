@@ -154,6 +154,13 @@ int phx_debug_enable_flux(phx_mesh* mesh, int on);
  * the face (i-1/2) stored at cell i), asynchronously on `stream`.  PHX_EINVAL for an inactive direction. */
 int phx_debug_flux(const phx_mesh* mesh, int d, double* d_out, void* stream);
 
+/* Failure detection ("guaranteed to always converge", 279-290 floors): the number of INTERIOR cells whose mask
+ * (as written by phx_cons_to_prim / phx_rk_stage / phx_rk2_step*) carries any of `bits` (PHX_M_*; e.g. PHX_M_NOCONV |
+ * PHX_M_BAD_INPUT for con2prim failures, PHX_M_RHO_FLOOR | PHX_M_EPS_FLOOR for the floors).  d_count (DEVICE, required) receives
+ * the count; h_count (HOST, nullable) also, with a stream synchronisation.  Excised cells carry PHX_M_EXCISED only. */
+int phx_count_masked(const phx_mesh* mesh, const unsigned char* d_mask, unsigned bits, unsigned long long* d_count,
+                     unsigned long long* h_count, void* stream);
+
 /* Count of this library's kernel launches since the mesh was created (for bench.py's gpu_launches). */
 unsigned long long phx_launch_count(const phx_mesh* mesh);
 

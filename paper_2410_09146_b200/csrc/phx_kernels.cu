@@ -1202,6 +1202,40 @@ extern "C" int phx_cfl_dt(const phx_mesh* M, const double* d_prim, double cfl, d
   return PHX_OK;
 }
 
+// ---- failure detection: how many interior cells carry any of the given mask bits ------------------------------------------
+__global__ void __launch_bounds__(256) k_count_masked(MeshDev m, const unsigned char* __restrict__ mask, unsigned bits,
+                                                      unsigned long long* __restrict__ count, long long ninterior) {
+  unsigned n = 0;
+  for (long long p = (long long)blockIdx.x * 256 + threadIdx.x; p < ninterior; p += (long long)gridDim.x * 256) {
+    const int ii = (int)(p % m.n[0]);
+    long long r = p / m.n[0];
+    const int jj = (int)(r % m.n[1]); r /= m.n[1];
+    const int kk = (int)(r % m.n[2]);
+    const int b = (int)(r / m.n[2]);
+    const long long c = (long long)b * m.ncell + (long long)(kk + m.g[2]) * m.sk + (long long)(jj + m.g[1]) * m.sj + (ii + m.g[0]);
+    n += (mask[c] & bits) != 0;
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) n += __shfl_xor_sync(0xffffffffu, n, o);
+  if ((threadIdx.x & 31) == 0 && n) atomicAdd(count, (unsigned long long)n);
+}
+
+extern "C" int phx_count_masked(const phx_mesh* M, const unsigned char* d_mask, unsigned bits, unsigned long long* d_count,
+                                unsigned long long* h_count, void* stream) {
+  if (!M || !d_mask || !d_count) return fail(PHX_EINVAL, "phx_count_masked: null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  CUDA_TRY(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), st), "cudaMemsetAsync");
+  long long want = (M->ninterior + 255) / 256;
+  const int nb = (int)(want < (long long)M->nsm * 8 ? want : (long long)M->nsm * 8);
+  k_count_masked<<<nb, 256, 0, st>>>(M->m, d_mask, bits, d_count, M->ninterior);
+  LAUNCH_CHECK(M, "k_count_masked");
+  if (h_count) {
+    CUDA_TRY(cudaMemcpyAsync(h_count, d_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st), "cudaMemcpyAsync");
+    CUDA_TRY(cudaStreamSynchronize(st), "cudaStreamSynchronize");
+  }
+  return PHX_OK;
+}
+
 // ---- per-kernel-class event timing ------------------------------------------------------------------------------
 extern "C" int phx_profile_enable(phx_mesh* M, int max_records) {
   if (!M || max_records < 0) return fail(PHX_EINVAL, "phx_profile_enable: null mesh or negative capacity");

@@ -26,7 +26,7 @@ EXPORTS = (
     "phx_cons_to_prim", "phx_fill_ghosts", "phx_rk_stage", "phx_cfl_dt", "phx_rk2_step",
     "phx_evolve_host", "phx_debug_flux", "phx_launch_count", "phx_last_error",
     "phx_profile_enable", "phx_profile_read", "phx_rk2_step_cfl", "phx_evolve_device", "phx_debug_enable_flux",
-    "phx_debug_fp64_peak",
+    "phx_debug_fp64_peak", "phx_count_masked",
 )
 
 
@@ -101,6 +101,7 @@ def lib():
         L.phx_profile_enable.argtypes = [vp, C.c_int]
         L.phx_profile_read.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(C.c_ulonglong)]
         L.phx_debug_fp64_peak.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(C.c_int), vp]
+        L.phx_count_masked.argtypes = [vp, ucp, C.c_uint, vp, C.POINTER(C.c_ulonglong), vp]
         L.phx_last_error.restype = C.c_char_p
         _lib = L
     return _lib
@@ -265,3 +266,13 @@ def debug_fp64_peak(min_seconds=0.5, stream=None):
     r, rb, ms, nsm = C.c_double(), C.c_double(), C.c_double(), C.c_int()
     _check(lib().phx_debug_fp64_peak(float(min_seconds), C.byref(r), C.byref(rb), C.byref(ms), C.byref(nsm), _stream(stream)))
     return r.value, rb.value, ms.value, nsm.value
+
+
+def count_masked(mesh, mask, bits, d_count=None, stream=None):
+    """Number of interior cells whose mask carries any of `bits` (synchronises the stream)."""
+    if d_count is None:
+        d_count = torch.zeros(1, dtype=torch.int64, device="cuda")
+    h = C.c_ulonglong(0)
+    _check(lib().phx_count_masked(mesh.handle, _dev(mask, torch.uint8, mesh.mask_elems, "mask"), int(bits),
+                                  _dev(d_count, torch.int64, 1, "d_count"), C.byref(h), _stream(stream)))
+    return h.value

@@ -55,3 +55,20 @@ def test_fp64_peak_measurement_is_sane():
     assert 150.0 < ms < 400.0
     nominal = nsm * 64 * 1.965e9              # one fp64 instruction per lane and cycle at the maximum SM clock
     assert 0.6 * nominal < rate <= 1.02 * nominal and 0.6 * nominal < burst <= 1.02 * nominal, (rate, burst, nominal)
+
+
+def test_count_masked_counts_interior_cells_only():
+    """phx_count_masked against numpy on a mesh whose floors act, with a poisoned ghost cell that must not be counted."""
+    import torch
+    w = wl.packed_blocks((2, 2, 2), 12)
+    g = GpuRun(w["params"], w["prim"])
+    g.step_device_dt(0.4)
+    p = w["params"]
+    m = g.mask.cpu().numpy()
+    gh = p["ng"]
+    inner = m[:, gh:-gh, gh:-gh, gh:-gh]
+    for bits in (64, 1 | 2, 255, 16 | 32):
+        assert g.phx.count_masked(g.mesh, g.mask, bits) == int(((inner & bits) != 0).sum())
+    assert g.phx.count_masked(g.mesh, g.mask, 64) > 0            # the excised cells of the torus recipe
+    g.mask[0, 0, 0, 0] = 255                                      # a ghost cell of the mask
+    assert g.phx.count_masked(g.mesh, g.mask, 255) == int((inner != 0).sum())
