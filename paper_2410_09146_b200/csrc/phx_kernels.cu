@@ -10,7 +10,8 @@
 //   k_update       flux-CT + accumulated divergence + geometric sources + RK combine + con2prim + floors, one thread per cell
 //   k_fill_ghosts  periodic / outflow / block-to-block ghost copies in one gather pass over the ghost cells
 // and k_cfl_partial / k_cfl_final (warp-shuffle min reduction), k_cfl_final_slots (fused into stage 2), k_prim_to_cons,
-// k_c2p, k_excision_flags, k_fp64_peak (the measured denominator of the ALU roofline); phx_evolve_device replays one captured
+// k_c2p, k_excision_flags, k_count_masked (failure detection), k_fp64_peak (the measured denominator of the ALU roofline);
+// phx_evolve_device replays one captured
 // step as a CUDA graph, or runs a small 1-D mesh entirely inside one thread block (k_evolve_1d).
 #include "phx_device.cuh"
 #include "../../include/phx.h"
@@ -1442,7 +1443,8 @@ __global__ void __launch_bounds__(SM1_MAXT, 1) k_evolve_1d(MeshDev m, int nsteps
 static bool small_1d_eligible(const phx_mesh* M) {
   const MeshDev& m = M->m;
   return m.nblk == 1 && m.act[0] && !m.act[1] && !m.act[2] && m.metric == 0 && m.nvar == NV && m.floor_form == 0 && !m.excise &&
-         m.n[0] + 2 <= SM1_MAXT && !M->store_all_fluxes && M->small_1d;
+         m.n[0] + 2 <= SM1_MAXT && 2 * m.g[0] <= ((m.n[0] + 2 + 31) / 32) * 32 &&   // one thread per cell, and per ghost cell in the fill
+         !M->store_all_fluxes && M->small_1d;
 }
 
 static int launch_evolve_1d(phx_mesh* M, int nsteps, double cfl, double* d_dt, double* d_t, double* d_cons0, double* d_cons, double* d_prim,
@@ -1450,9 +1452,10 @@ static int launch_evolve_1d(phx_mesh* M, int nsteps, double cfl, double* d_dt, d
   const MeshDev& m = M->m;
   const int threads = ((m.n[0] + 2 + 31) / 32) * 32;
   const size_t smem = 2 * NV * SM1_MAXT * sizeof(double);
-#define EV1(REC) case REC: { static bool once = false; \
-    if (!once) { CUDA_TRY(cudaFuncSetAttribute(k_evolve_1d<REC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "cudaFuncSetAttribute"); once = true; } \
-    k_evolve_1d<REC><<<1, threads, smem, st>>>(m, nsteps, cfl, d_dt, d_t, d_cons0, d_cons, d_prim, d_mask); } break;
+  // 128 KB of dynamic shared memory need the opt-in of the kernel attribute (per device and context: set on every call)
+#define EV1(REC) case REC: \
+    CUDA_TRY(cudaFuncSetAttribute(k_evolve_1d<REC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), "cudaFuncSetAttribute"); \
+    k_evolve_1d<REC><<<1, threads, smem, st>>>(m, nsteps, cfl, d_dt, d_t, d_cons0, d_cons, d_prim, d_mask); break;
   switch (m.recon) {
     EV1(0) EV1(1) EV1(2) EV1(3) EV1(4) EV1(5)
     default: return fail(PHX_EUNSUPPORTED, "k_evolve_1d: unknown reconstruction");
